@@ -1,0 +1,119 @@
+/*
+ * plspec.h -- C ABI of the B200-native plasma-line spectral integrator.
+ *
+ * One operation (arXiv 2311.18737, "GPGPU Acceleration of Incoherent Scatter Radar Plasma
+ * Line Analysis"; citations are PAPER.md line numbers + section):
+ *
+ *   for every inter-pulse period (IPP) p and range gate r
+ *       d[t]    = V[p][r0 + r*stride + t] * conj(C[p][t])   t <  code_len   (sec. 3.2.1)
+ *               = 0                                          code_len <= t < N
+ *       X[f]    = sum_{t<N} d[t] * exp(-2*pi*i*f*t/N)                         (sec. 3.2.2)
+ *       S[r][f] += |X[f]|^2 = Re^2 + Im^2                                     (Eq. 8, 113-115 sec. 3.2.3)
+ *   summed over every IPP given since create / the last finalize             (sec. 3.2.4)
+ *
+ * Un-normalised forward FFT, plain sum over IPPs (no 1/N, no 1/P), natural bin order with
+ * DC at f = 0.  All arithmetic runs in fp32 CUDA kernels (sm_100a); there is no CPU path.
+ *
+ * Conventions
+ *   - Every function returns an int status: PLSPEC_OK (0) or a negative PLSPEC_ERR_*.
+ *     Nothing is printed, thrown or aborted across this boundary.
+ *   - Pointers marked [host] are host pointers; [device] are CUDA device pointers on the
+ *     device that was current at plspec_create; [host|device] may be either (detected with
+ *     cudaPointerGetAttributes).
+ *   - The caller owns every buffer it passes.  The library owns the handle and everything
+ *     behind it (accumulators, tables, staging buffers, streams) until plspec_destroy.
+ *   - A handle is not thread-safe; distinct handles are independent.
+ */
+#ifndef PLSPEC_H
+#define PLSPEC_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct plspec_ctx *plspec_handle;   /* opaque, library-owned */
+
+/* dtype of `voltages` (codes are always interleaved float32 re,im). */
+enum { PLSPEC_CF32 = 0,    /* interleaved float32 (re, im), 8 bytes / sample                    */
+       PLSPEC_SC16 = 1 };  /* interleaved little-endian int16 (I, Q), 4 bytes / sample, converted
+                              exactly on the device, NO 1/32768 scaling (S is in counts^2)      */
+
+enum { PLSPEC_OK = 0,
+       PLSPEC_ERR_INVALID_ARG = -1,  /* bad argument; no state changed                          */
+       PLSPEC_ERR_ALLOC       = -2,  /* host or device allocation failed                        */
+       PLSPEC_ERR_CUDA        = -3,  /* a CUDA call failed; see plspec_last_cuda_error          */
+       PLSPEC_ERR_UNSUPPORTED = -4 };/* valid request this build cannot serve (e.g. not sm_100) */
+
+/* plspec_configure options (EXTENSION; defaults in brackets). */
+enum { PLSPEC_OPT_KERNEL     = 1,   /* [0] 0 = auto, 1 = generic radix-2 kernel, 2 = fused kernel   */
+       PLSPEC_OPT_IPP_CHUNKS = 2,   /* [0] 0 = auto; else split each accumulate's IPPs over this many
+                                       CTAs per gate (partial sums meet in S with fp32 atomics)     */
+       PLSPEC_OPT_H2D_BATCH  = 3 }; /* [0] 0 = auto; IPPs per host->device staging batch            */
+
+/* Counters since create (EXTENSION; used by bench.py for gpu_launches / h2d bytes). */
+typedef struct {
+    long long kernel_launches;   /* kernels of this library launched                       */
+    long long h2d_bytes;         /* bytes copied host->device by plspec_accumulate          */
+    long long d2h_bytes;         /* bytes copied device->host by plspec_finalize            */
+    long long ipps_accumulated;  /* IPPs accumulated since create                           */
+    int       kernel_kind;       /* 1 = generic, 2 = fused (what `auto` resolved to)        */
+    int       ipp_chunks_last;   /* IPP chunks per gate used by the last accumulate         */
+} plspec_stats_t;
+
+/*
+ * Create an integrator.  ("iterating through the number of range gates we desire
+ * and the amount to step each of them"; "4096 range gates with a step size of 25,
+ * starting at the first element"; PAPER.md:111 power-of-two row length.)
+ *   N         FFT length, a power of two in [16, 65536]
+ *   code_len  samples per transmit code, 1 <= code_len <= N (shorter codes are zero-padded to N)
+ *   n_ranges  number of range gates R >= 1
+ *   r0        first sample of gate 0 within an IPP, >= 0
+ *   stride    samples between successive gates, >= 1
+ *   ipp_len   EXTENSION: samples per IPP row of `voltages` (the pitch); 0 means the tightly
+ *             packed span r0 + (R-1)*stride + code_len.  The span must fit in ipp_len.
+ *   dtype     PLSPEC_CF32 or PLSPEC_SC16
+ *   out       [host] receives the handle; NULL on any error
+ * Allocates S_dev[R][N] fp32 on the current device (zeroed) and the twiddle tables.
+ */
+int plspec_create(int N, int code_len, int n_ranges, int r0, int stride, int ipp_len,
+                  int dtype, plspec_handle *out);
+
+/*
+ * Accumulate n_ipp pulses: S[r][f] += |FFT_N(decode(p, r))[f]|^2 for every gate r.
+ *   voltages  [host|device] voltages[n_ipp][ipp_len], element per dtype, C-contiguous
+ *   codes     [host|device] codes[n_ipp][code_len], interleaved float32 (re, im); one code per
+ *             IPP ("a single full TX and echo" per pulse)
+ *   n_ipp     >= 0; 0 is a successful no-op
+ *   stream    cudaStream_t to order the work on (NULL = the legacy default stream)
+ * Device pointers: the fused kernel is enqueued on `stream` and the call returns without
+ * synchronising; the buffers must stay valid until that stream work completes.
+ * Host pointers: the needed span of each IPP (not the whole row: PAPER.md:149 item 3) and its
+ * code are copied in batches on an internal copy stream, overlapped with compute on `stream`
+ * (PAPER.md:149 item 2).  Pinned buffers make the copies asynchronous; they must stay valid
+ * until plspec_finalize (or a synchronisation of `stream`).  Pageable buffers work but the
+ * copies are staged synchronously by the driver.  Both pointers must be of the same kind.
+ */
+int plspec_accumulate(plspec_handle h, const void *voltages, const void *codes,
+                      int n_ipp, void *stream);
+
+/*
+ * Finish an integration: wait for all accumulate work, write S_out[n_ranges][N] (fp32,
+ * row-major, natural FFT bin order, un-normalised sum) and zero the accumulators so the next
+ * integration starts clean ("Upon completion, we transfer the spectrum result
+ * back").  S_out is [host|device]; the call blocks until S_out is complete.
+ */
+int plspec_finalize(plspec_handle h, float *S_out);
+
+/* EXTENSIONS ------------------------------------------------------------------------------- */
+int plspec_reset(plspec_handle h);                        /* zero the accumulators, no output */
+int plspec_destroy(plspec_handle h);                      /* free everything; NULL is OK       */
+int plspec_configure(plspec_handle h, int option, int value);
+int plspec_get_stats(plspec_handle h, plspec_stats_t *out /* [host] */);
+int plspec_last_cuda_error(plspec_handle h);              /* cudaError_t of the last failure   */
+const char *plspec_strerror(int status);                  /* static string, never NULL         */
+const char *plspec_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PLSPEC_H */

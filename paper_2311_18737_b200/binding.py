@@ -1,0 +1,222 @@
+"""Thin ctypes binding of libplspec.so -- same names as include/plspec.h.
+
+Argument marshalling only: every step of the path (sc16 conversion, decode, FFT, |X|^2,
+accumulation, write-out) runs in the CUDA kernels behind the C ABI.  There is no CPU
+fallback: if the library is missing or fails to load, importing callers get an exception.
+
+Buffers may be torch tensors (CUDA or CPU, pinned or not) or numpy arrays (host); the
+binding passes their raw pointers.  PyTorch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+PLSPEC_CF32 = 0
+PLSPEC_SC16 = 1
+
+PLSPEC_OK = 0
+PLSPEC_ERR_INVALID_ARG = -1
+PLSPEC_ERR_ALLOC = -2
+PLSPEC_ERR_CUDA = -3
+PLSPEC_ERR_UNSUPPORTED = -4
+
+PLSPEC_OPT_KERNEL = 1
+PLSPEC_OPT_IPP_CHUNKS = 2
+PLSPEC_OPT_H2D_BATCH = 3
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_FUSED = 0, 1, 2
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libplspec.so")
+
+# every symbol include/plspec.h declares (tests check the library exports each one)
+EXPORTED_SYMBOLS = (
+    "plspec_create", "plspec_accumulate", "plspec_finalize", "plspec_reset", "plspec_destroy",
+    "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_strerror",
+    "plspec_version",
+)
+
+
+class plspec_stats_t(ctypes.Structure):
+    _fields_ = [
+        ("kernel_launches", ctypes.c_longlong),
+        ("h2d_bytes", ctypes.c_longlong),
+        ("d2h_bytes", ctypes.c_longlong),
+        ("ipps_accumulated", ctypes.c_longlong),
+        ("kernel_kind", ctypes.c_int),
+        ("ipp_chunks_last", ctypes.c_int),
+    ]
+
+
+class PlspecError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda_error: int = 0):
+        self.status = status
+        self.cuda_error = cuda_error
+        msg = f"{where}: {strerror(status)} (status {status}"
+        msg += f", cudaError {cuda_error})" if cuda_error else ")"
+        super().__init__(msg)
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libplspec.so (built in-tree by paper_2311_18737_b200.build). Fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2311_18737_b200.build` "
+                "(nvcc, sm_100a). There is no CPU fallback.")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci = ctypes.c_void_p, ctypes.c_int
+        L.plspec_create.argtypes = [ci, ci, ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
+        L.plspec_accumulate.argtypes = [vp, vp, vp, ci, vp]
+        L.plspec_finalize.argtypes = [vp, vp]
+        L.plspec_reset.argtypes = [vp]
+        L.plspec_destroy.argtypes = [vp]
+        L.plspec_configure.argtypes = [vp, ci, ci]
+        L.plspec_get_stats.argtypes = [vp, ctypes.POINTER(plspec_stats_t)]
+        L.plspec_last_cuda_error.argtypes = [vp]
+        L.plspec_strerror.argtypes = [ci]
+        L.plspec_strerror.restype = ctypes.c_char_p
+        L.plspec_version.restype = ctypes.c_char_p
+        for name in EXPORTED_SYMBOLS[:8]:
+            getattr(L, name).restype = ci
+        _lib = L
+    return _lib
+
+
+def strerror(status: int) -> str:
+    try:
+        return lib().plspec_strerror(int(status)).decode()
+    except Exception:
+        return f"status {status}"
+
+
+def _ptr(buf) -> int:
+    """Raw address of a torch tensor / numpy array / int; contiguity is the caller's duty."""
+    if buf is None:
+        return 0
+    if isinstance(buf, int):
+        return buf
+    if hasattr(buf, "data_ptr"):
+        if not buf.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return int(buf.data_ptr())
+    if isinstance(buf, np.ndarray):
+        if not buf.flags.c_contiguous:
+            raise ValueError("array must be C-contiguous")
+        return int(buf.ctypes.data)
+    raise TypeError(f"unsupported buffer type {type(buf)}")
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        return 0
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)          # torch.cuda.Stream
+
+
+# ---- the C calls, one to one -----------------------------------------------------------------
+def plspec_create(N, code_len, n_ranges, r0, stride, ipp_len, dtype) -> int:
+    h = ctypes.c_void_p()
+    rc = lib().plspec_create(N, code_len, n_ranges, r0, stride, ipp_len, dtype, ctypes.byref(h))
+    if rc != PLSPEC_OK:
+        raise PlspecError(rc, "plspec_create")
+    return h.value
+
+
+def _check(h, rc, where):
+    if rc != PLSPEC_OK:
+        raise PlspecError(rc, where, lib().plspec_last_cuda_error(h) if h else 0)
+
+
+def plspec_accumulate(h, voltages, codes, n_ipp, stream=None) -> None:
+    _check(h, lib().plspec_accumulate(h, _ptr(voltages), _ptr(codes), int(n_ipp), _stream_ptr(stream)),
+           "plspec_accumulate")
+
+
+def plspec_finalize(h, S_out) -> None:
+    _check(h, lib().plspec_finalize(h, _ptr(S_out)), "plspec_finalize")
+
+
+def plspec_reset(h) -> None:
+    _check(h, lib().plspec_reset(h), "plspec_reset")
+
+
+def plspec_destroy(h) -> None:
+    lib().plspec_destroy(h)
+
+
+def plspec_configure(h, option, value) -> None:
+    _check(h, lib().plspec_configure(h, int(option), int(value)), "plspec_configure")
+
+
+def plspec_get_stats(h) -> dict:
+    st = plspec_stats_t()
+    _check(h, lib().plspec_get_stats(h, ctypes.byref(st)), "plspec_get_stats")
+    return {k: getattr(st, k) for k, _ in plspec_stats_t._fields_}
+
+
+def plspec_version() -> str:
+    return lib().plspec_version().decode()
+
+
+# ---- convenience wrapper (lifetime only; no arithmetic) ---------------------------------------
+class Integrator:
+    """Owns one plspec handle.  `accumulate` / `finalize` forward to the C calls."""
+
+    def __init__(self, N, code_len, n_ranges, r0=0, stride=1, ipp_len=0, dtype=PLSPEC_CF32,
+                 kernel=KERNEL_AUTO, ipp_chunks=0, h2d_batch=0):
+        self.N, self.n_ranges = N, n_ranges
+        self.h = plspec_create(N, code_len, n_ranges, r0, stride, ipp_len, dtype)
+        try:
+            if kernel:
+                plspec_configure(self.h, PLSPEC_OPT_KERNEL, kernel)
+            if ipp_chunks:
+                plspec_configure(self.h, PLSPEC_OPT_IPP_CHUNKS, ipp_chunks)
+            if h2d_batch:
+                plspec_configure(self.h, PLSPEC_OPT_H2D_BATCH, h2d_batch)
+        except Exception:
+            self.close()
+            raise
+
+    @classmethod
+    def for_workload(cls, w, **kw):
+        return cls(w.N, w.code_len, w.n_ranges, w.r0, w.stride, w.ipp_len, w.dtype, **kw)
+
+    def accumulate(self, voltages, codes, n_ipp=None, stream=None):
+        if n_ipp is None:
+            n_ipp = int(codes.shape[0])
+        plspec_accumulate(self.h, voltages, codes, n_ipp, stream)
+
+    def finalize(self, S_out):
+        plspec_finalize(self.h, S_out)
+        return S_out
+
+    def reset(self):
+        plspec_reset(self.h)
+
+    def stats(self):
+        return plspec_get_stats(self.h)
+
+    def close(self):
+        if getattr(self, "h", None):
+            plspec_destroy(self.h)
+            self.h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,447 @@
+// plspec_api.cu -- C ABI (include/plspec.h), handle, validation, launch logic and the
+// multi-stream host loop.  No CPU compute path exists: every
+// step of decode / FFT / power / accumulate runs in the kernels of plspec_kernels.cuh.
+#include "../../include/plspec.h"
+#include "plspec_kernels.cuh"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace plspec;
+
+namespace {
+
+constexpr int kSlots = 3;            // host->device staging ring depth
+constexpr int kMaxNk = 16384;        // largest window one SM holds (fused and generic kernels)
+
+struct Slot {
+    void   *V = nullptr;             // [batch][span] voltages (storage dtype)
+    float2 *C = nullptr;             // [batch][L]
+    cudaEvent_t ready = nullptr;     // copies into the slot finished   (recorded on copy stream)
+    cudaEvent_t freed = nullptr;     // kernel reading the slot finished (recorded on compute stream)
+    bool used = false;
+};
+
+}  // namespace
+
+struct plspec_ctx {
+    int N, L, R, r0, stride, ipp_len, dtype;
+    int span;                        // (R-1)*stride + L samples needed from r0 on
+    int device = 0, n_sm = 0;
+    // kernel selection
+    int kind = 2;                    // 1 generic, 2 fused
+    int Nk = 0, Q = 1, R3 = 1;
+    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0;
+    int block = 0;
+    size_t smem = 0;
+    int slots_per_wave = 0;          // n_sm * resident CTAs per SM
+    const void *kfunc = nullptr;
+    // device state
+    float  *S = nullptr;             // [R][Q][Nk]
+    float  *S_tmp = nullptr;         // interleave target when S_out is a host pointer and Q > 1
+    float2 *tw1 = nullptr, *twN = nullptr;
+    // host pipeline
+    cudaStream_t copy_stream = nullptr;
+    Slot slot[kSlots];
+    int slot_batch = 0;              // IPPs each slot can hold
+    int next_slot = 0;
+    // ordering
+    cudaEvent_t work_done = nullptr;
+    cudaStream_t last_stream = nullptr;
+    bool have_work = false;
+    // bookkeeping
+    int last_cuda = 0;
+    plspec_stats_t stats;
+};
+
+namespace {
+
+#define PL_CUDA(h, call)                                                   \
+    do {                                                                   \
+        cudaError_t e__ = (call);                                          \
+        if (e__ != cudaSuccess) {                                          \
+            if (h) (h)->last_cuda = (int)e__;                              \
+            (void)cudaGetLastError();                                      \
+            return PLSPEC_ERR_CUDA;                                        \
+        }                                                                  \
+    } while (0)
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+template <int R3, int Q>
+const void *fused_ptr(int dt) {
+    return dt == DT_CF32 ? (const void *)fused_kernel<R3, Q, DT_CF32>
+                         : (const void *)fused_kernel<R3, Q, DT_SC16>;
+}
+// the outer radix Q > 1 only occurs with the largest inner size (Nk = 16384, R3 = 16)
+const void *fused_lookup(int R3, int Q, int dt) {
+    if (Q == 1) {
+        switch (R3) {
+            case 1:  return fused_ptr<1, 1>(dt);
+            case 2:  return fused_ptr<2, 1>(dt);
+            case 4:  return fused_ptr<4, 1>(dt);
+            case 8:  return fused_ptr<8, 1>(dt);
+            case 16: return fused_ptr<16, 1>(dt);
+        }
+    } else if (R3 == 16) {
+        if (Q == 2) return fused_ptr<16, 2>(dt);
+        if (Q == 4) return fused_ptr<16, 4>(dt);
+    }
+    return nullptr;
+}
+
+bool g_tw2_ready[64] = {false};
+
+int upload_tw2(plspec_ctx *h) {
+    if (h->device < 64 && g_tw2_ready[h->device]) return PLSPEC_OK;
+    std::vector<float2> t(960);
+    for (int R3 = 2; R3 <= 16; R3 *= 2) {
+        const int M1 = 32 * R3;
+        for (int t3 = 0; t3 < R3; t3++)
+            for (int f2 = 0; f2 < 32; f2++) {
+                double a = -2.0 * M_PI * (double)((t3 * f2) % M1) / (double)M1;
+                t[tw2_offset(R3) + t3 * 32 + f2] = make_float2((float)cos(a), (float)sin(a));
+            }
+    }
+    PL_CUDA(h, cudaMemcpyToSymbol(c_tw2, t.data(), sizeof(float2) * 960));
+    if (h->device < 64) g_tw2_ready[h->device] = true;
+    return PLSPEC_OK;
+}
+
+// Resolve kernel kind / geometry from N and the options; (re)build what depends on it.
+int select_kernel(plspec_ctx *h) {
+    int kind = h->opt_kernel ? h->opt_kernel : (h->N >= 1024 ? 2 : 1);
+    if (kind == 2 && h->N < 1024) return PLSPEC_ERR_UNSUPPORTED;
+    h->kind = kind;
+    h->Nk = h->N < kMaxNk ? h->N : kMaxNk;
+    h->Q = h->N / h->Nk;
+    const int dt = h->dtype == PLSPEC_SC16 ? DT_SC16 : DT_CF32;
+    if (kind == 2) {
+        h->R3 = h->Nk / 1024;
+        h->block = 32 * h->R3;
+        h->smem = (size_t)h->block * 33 * sizeof(float2);
+        h->kfunc = fused_lookup(h->R3, h->Q, dt);
+    } else {
+        h->R3 = 0;
+        h->block = h->Nk / 2 < 32 ? 32 : (h->Nk / 2 > 512 ? 512 : h->Nk / 2);
+        h->smem = (size_t)h->Nk * (sizeof(float2) + sizeof(float));
+        h->kfunc = dt == DT_CF32 ? (const void *)generic_kernel<DT_CF32> : (const void *)generic_kernel<DT_SC16>;
+    }
+    if (!h->kfunc) return PLSPEC_ERR_UNSUPPORTED;
+    PL_CUDA(h, cudaFuncSetAttribute(h->kfunc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem));
+    int occ = 0;
+    PL_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->kfunc, h->block, h->smem));
+    if (occ < 1) return PLSPEC_ERR_UNSUPPORTED;
+    h->slots_per_wave = occ * h->n_sm;
+    h->stats.kernel_kind = kind;
+    return PLSPEC_OK;
+}
+
+// IPP chunks per (gate, q): more CTAs than one wave can hold, whole waves, few flushes.
+int pick_chunks(const plspec_ctx *h, int n_ipp) {
+    if (h->opt_chunks > 0) return h->opt_chunks < n_ipp ? h->opt_chunks : n_ipp;
+    const long long base = (long long)h->R * h->Q;
+    const int slots = h->slots_per_wave;
+    int best = 1;
+    double best_score = -1.0;
+    for (int c = 1; c <= n_ipp && c <= 64; c++) {
+        const long long tiles = base * c;
+        const long long waves = (tiles + slots - 1) / slots;
+        const double eff = (double)tiles / (double)(waves * slots);
+        const double per = (double)n_ipp / c;            // IPPs per chunk; a flush costs ~half a window
+        const double score = eff * per / (per + 0.5);
+        if (score > best_score + 1e-9) { best_score = score; best = c; }
+    }
+    return best;
+}
+
+int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0,
+                      int n_ipp, cudaStream_t stream) {
+    KParams P;
+    P.V = dV; P.C = dC; P.S = h->S; P.tw1 = h->tw1; P.twN = h->twN;
+    P.v_pitch = v_pitch;
+    P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
+    P.L = h->L; P.R = h->R; P.r0 = r0; P.stride = h->stride;
+    P.n_ipp = n_ipp;
+    P.n_chunks = pick_chunks(h, n_ipp);
+    P.use_atomic = P.n_chunks > 1 ? 1 : 0;
+    h->stats.ipp_chunks_last = P.n_chunks;
+    const long long tiles = (long long)h->R * h->Q * P.n_chunks;
+    if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
+    void *args[] = {&P};
+    PL_CUDA(h, cudaLaunchKernel(h->kfunc, dim3((unsigned)tiles), dim3((unsigned)h->block), args, h->smem, stream));
+    h->stats.kernel_launches++;
+    return PLSPEC_OK;
+}
+
+// order this call's work after everything accumulated before on another stream
+int chain_streams(plspec_ctx *h, cudaStream_t stream) {
+    if (h->have_work && h->last_stream != stream) PL_CUDA(h, cudaStreamWaitEvent(stream, h->work_done, 0));
+    return PLSPEC_OK;
+}
+int mark_work(plspec_ctx *h, cudaStream_t stream) {
+    PL_CUDA(h, cudaEventRecord(h->work_done, stream));
+    h->last_stream = stream;
+    h->have_work = true;
+    return PLSPEC_OK;
+}
+
+int ensure_slots(plspec_ctx *h, int batch) {
+    if (h->slot_batch >= batch) return PLSPEC_OK;
+    const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
+    for (int s = 0; s < kSlots; s++) {
+        Slot &sl = h->slot[s];
+        if (sl.used) PL_CUDA(h, cudaEventSynchronize(sl.freed));
+        if (sl.V) cudaFree(sl.V);
+        if (sl.C) cudaFree(sl.C);
+        sl.V = nullptr; sl.C = nullptr; sl.used = false;
+        if (cudaMalloc(&sl.V, (size_t)batch * h->span * esz) != cudaSuccess ||
+            cudaMalloc((void **)&sl.C, (size_t)batch * h->L * sizeof(float2)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            h->slot_batch = 0;
+            return PLSPEC_ERR_ALLOC;
+        }
+        if (!sl.ready) PL_CUDA(h, cudaEventCreateWithFlags(&sl.ready, cudaEventDisableTiming));
+        if (!sl.freed) PL_CUDA(h, cudaEventCreateWithFlags(&sl.freed, cudaEventDisableTiming));
+    }
+    h->slot_batch = batch;
+    return PLSPEC_OK;
+}
+
+// Host-resident inputs: copy only the needed span of each IPP (PAPER.md:149 item 3) in batches
+// on the copy stream, overlapped with the kernels of earlier batches (PAPER.md:149 item 2).
+int accumulate_from_host(plspec_ctx *h, const void *V, const void *C, int n_ipp, cudaStream_t stream) {
+    const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
+    int batch = h->opt_batch > 0 ? h->opt_batch : (n_ipp + 7) / 8;
+    const size_t per_ipp = (size_t)h->span * esz + (size_t)h->L * sizeof(float2);
+    const int cap = (int)((256u << 20) / per_ipp);        // <= 256 MiB per slot
+    if (batch > cap) batch = cap;
+    if (batch < 1) batch = 1;
+    if (batch > n_ipp) batch = n_ipp;
+    int rc = ensure_slots(h, batch);
+    if (rc) return rc;
+    for (int p0 = 0; p0 < n_ipp; p0 += batch) {
+        const int nb = n_ipp - p0 < batch ? n_ipp - p0 : batch;
+        Slot &sl = h->slot[h->next_slot];
+        h->next_slot = (h->next_slot + 1) % kSlots;
+        if (sl.used) PL_CUDA(h, cudaStreamWaitEvent(h->copy_stream, sl.freed, 0));
+        const char *src = (const char *)V + ((size_t)p0 * h->ipp_len + h->r0) * esz;
+        PL_CUDA(h, cudaMemcpy2DAsync(sl.V, (size_t)h->span * esz, src, (size_t)h->ipp_len * esz,
+                                     (size_t)h->span * esz, nb, cudaMemcpyHostToDevice, h->copy_stream));
+        PL_CUDA(h, cudaMemcpyAsync(sl.C, (const char *)C + (size_t)p0 * h->L * sizeof(float2),
+                                   (size_t)nb * h->L * sizeof(float2), cudaMemcpyHostToDevice, h->copy_stream));
+        h->stats.h2d_bytes += (long long)nb * (long long)per_ipp;
+        PL_CUDA(h, cudaEventRecord(sl.ready, h->copy_stream));
+        PL_CUDA(h, cudaStreamWaitEvent(stream, sl.ready, 0));
+        rc = launch_accumulate(h, sl.V, sl.C, h->span, 0, nb, stream);
+        if (rc) return rc;
+        PL_CUDA(h, cudaEventRecord(sl.freed, stream));
+        sl.used = true;
+    }
+    return PLSPEC_OK;
+}
+
+int build_tables(plspec_ctx *h) {
+    // full circle W_N^e, correctly rounded from float64 (never a recurrence)
+    std::vector<float2> t((size_t)h->N);
+    for (int e = 0; e < h->N; e++) {
+        double a = -2.0 * M_PI * (double)e / (double)h->N;
+        t[e] = make_float2((float)cos(a), (float)sin(a));
+    }
+    PL_CUDA(h, cudaMalloc((void **)&h->twN, sizeof(float2) * (size_t)h->N));
+    PL_CUDA(h, cudaMemcpy(h->twN, t.data(), sizeof(float2) * (size_t)h->N, cudaMemcpyHostToDevice));
+    // pass-1 -> pass-2 twiddles of the fused kernel: [f1][n'] = W_Nk^{f1 n'}
+    const int Nk = h->N < kMaxNk ? h->N : kMaxNk;
+    if (Nk >= 1024) {
+        const int M1 = Nk / 32;
+        std::vector<float2> u((size_t)Nk);
+        for (int f1 = 0; f1 < 32; f1++)
+            for (int n = 0; n < M1; n++) {
+                double a = -2.0 * M_PI * (double)(((long long)f1 * n) % Nk) / (double)Nk;
+                u[(size_t)f1 * M1 + n] = make_float2((float)cos(a), (float)sin(a));
+            }
+        PL_CUDA(h, cudaMalloc((void **)&h->tw1, sizeof(float2) * (size_t)Nk));
+        PL_CUDA(h, cudaMemcpy(h->tw1, u.data(), sizeof(float2) * (size_t)Nk, cudaMemcpyHostToDevice));
+    }
+    return upload_tw2(h);
+}
+
+void free_ctx(plspec_ctx *h) {
+    if (!h) return;
+    (void)cudaDeviceSynchronize();
+    for (int s = 0; s < kSlots; s++) {
+        if (h->slot[s].V) cudaFree(h->slot[s].V);
+        if (h->slot[s].C) cudaFree(h->slot[s].C);
+        if (h->slot[s].ready) cudaEventDestroy(h->slot[s].ready);
+        if (h->slot[s].freed) cudaEventDestroy(h->slot[s].freed);
+    }
+    if (h->S) cudaFree(h->S);
+    if (h->S_tmp) cudaFree(h->S_tmp);
+    if (h->tw1) cudaFree(h->tw1);
+    if (h->twN) cudaFree(h->twN);
+    if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+    if (h->work_done) cudaEventDestroy(h->work_done);
+    (void)cudaGetLastError();
+    delete h;
+}
+
+// 1 = device-accessible (device / managed), 0 = host (pinned or pageable), <0 error
+int pointer_is_device(plspec_ctx *h, const void *p, int *is_dev) {
+    cudaPointerAttributes a;
+    cudaError_t e = cudaPointerGetAttributes(&a, p);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); h->last_cuda = (int)e; return PLSPEC_ERR_CUDA; }
+    *is_dev = (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged) ? 1 : 0;
+    return PLSPEC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int plspec_create(int N, int code_len, int n_ranges, int r0, int stride, int ipp_len, int dtype,
+                  plspec_handle *out) {
+    if (!out) return PLSPEC_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!is_pow2(N) || N < 16 || N > 65536) return PLSPEC_ERR_INVALID_ARG;
+    if (code_len < 1 || code_len > N || n_ranges < 1 || r0 < 0 || stride < 1 || ipp_len < 0)
+        return PLSPEC_ERR_INVALID_ARG;
+    if (dtype != PLSPEC_CF32 && dtype != PLSPEC_SC16) return PLSPEC_ERR_INVALID_ARG;
+    const long long span = (long long)(n_ranges - 1) * stride + code_len;
+    if (span + r0 > 0x7fffffffLL) return PLSPEC_ERR_INVALID_ARG;
+    if (ipp_len == 0) ipp_len = (int)(span + r0);
+    if (span + r0 > ipp_len) return PLSPEC_ERR_INVALID_ARG;
+
+    plspec_ctx *h = new (std::nothrow) plspec_ctx();
+    if (!h) return PLSPEC_ERR_ALLOC;
+    memset(&h->stats, 0, sizeof(h->stats));
+    h->N = N; h->L = code_len; h->R = n_ranges; h->r0 = r0; h->stride = stride;
+    h->ipp_len = ipp_len; h->dtype = dtype; h->span = (int)span;
+
+    int rc = PLSPEC_OK;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDevice(&h->device);
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, h->device);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); delete h; return PLSPEC_ERR_CUDA; }
+    if (prop.major < 10) { delete h; return PLSPEC_ERR_UNSUPPORTED; }   // sm_100a code only
+    h->n_sm = prop.multiProcessorCount;
+
+    auto fail = [&](int code) { free_ctx(h); return code; };
+    const size_t s_bytes = sizeof(float) * (size_t)n_ranges * (size_t)N;
+    if (cudaMalloc((void **)&h->S, s_bytes) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_ALLOC); }
+    if (cudaMemset(h->S, 0, s_bytes) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_CUDA); }
+    if (cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->work_done, cudaEventDisableTiming) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return fail(PLSPEC_ERR_CUDA);
+    }
+    if ((rc = build_tables(h)) != PLSPEC_OK) return fail(rc);
+    if ((rc = select_kernel(h)) != PLSPEC_OK) return fail(rc);
+    *out = h;
+    return PLSPEC_OK;
+}
+
+int plspec_configure(plspec_handle h, int option, int value) {
+    if (!h || value < 0) return PLSPEC_ERR_INVALID_ARG;
+    switch (option) {
+        case PLSPEC_OPT_KERNEL: {
+            if (value > 2) return PLSPEC_ERR_INVALID_ARG;
+            const int old = h->opt_kernel;
+            h->opt_kernel = value;
+            int rc = select_kernel(h);
+            if (rc != PLSPEC_OK) { h->opt_kernel = old; (void)select_kernel(h); }
+            return rc;
+        }
+        case PLSPEC_OPT_IPP_CHUNKS: h->opt_chunks = value; return PLSPEC_OK;
+        case PLSPEC_OPT_H2D_BATCH:  h->opt_batch = value;  return PLSPEC_OK;
+    }
+    return PLSPEC_ERR_INVALID_ARG;
+}
+
+int plspec_accumulate(plspec_handle h, const void *voltages, const void *codes, int n_ipp, void *stream_) {
+    if (!h || n_ipp < 0) return PLSPEC_ERR_INVALID_ARG;
+    if (n_ipp == 0) return PLSPEC_OK;
+    if (!voltages || !codes) return PLSPEC_ERR_INVALID_ARG;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    int vdev = 0, cdev = 0, rc;
+    if ((rc = pointer_is_device(h, voltages, &vdev)) != PLSPEC_OK) return rc;
+    if ((rc = pointer_is_device(h, codes, &cdev)) != PLSPEC_OK) return rc;
+    if (vdev != cdev) return PLSPEC_ERR_INVALID_ARG;
+    if ((rc = chain_streams(h, stream)) != PLSPEC_OK) return rc;
+    if (vdev) rc = launch_accumulate(h, voltages, (const float2 *)codes, h->ipp_len, h->r0, n_ipp, stream);
+    else      rc = accumulate_from_host(h, voltages, codes, n_ipp, stream);
+    if (rc != PLSPEC_OK) return rc;
+    h->stats.ipps_accumulated += n_ipp;
+    return mark_work(h, stream);
+}
+
+int plspec_finalize(plspec_handle h, float *S_out) {
+    if (!h || !S_out) return PLSPEC_ERR_INVALID_ARG;
+    int out_dev = 0, rc;
+    if ((rc = pointer_is_device(h, S_out, &out_dev)) != PLSPEC_OK) return rc;
+    cudaStream_t st = h->last_stream;
+    const size_t total = (size_t)h->R * (size_t)h->N;
+    const float *src = h->S;
+    if (h->Q > 1) {
+        float *dst = S_out;
+        if (!out_dev) {
+            if (!h->S_tmp && cudaMalloc((void **)&h->S_tmp, total * sizeof(float)) != cudaSuccess) {
+                (void)cudaGetLastError();
+                return PLSPEC_ERR_ALLOC;
+            }
+            dst = h->S_tmp;
+        }
+        interleave_kernel<<<h->n_sm * 8, 256, 0, st>>>(h->S, dst, h->Q, h->Nk, (long long)total);
+        PL_CUDA(h, cudaGetLastError());
+        h->stats.kernel_launches++;
+        src = dst;
+    }
+    if (src != S_out) {
+        PL_CUDA(h, cudaMemcpyAsync(S_out, src, total * sizeof(float),
+                                   out_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+        if (!out_dev) h->stats.d2h_bytes += (long long)(total * sizeof(float));
+    }
+    PL_CUDA(h, cudaMemsetAsync(h->S, 0, total * sizeof(float), st));
+    PL_CUDA(h, cudaStreamSynchronize(st));
+    h->have_work = false;
+    return PLSPEC_OK;
+}
+
+int plspec_reset(plspec_handle h) {
+    if (!h) return PLSPEC_ERR_INVALID_ARG;
+    cudaStream_t st = h->last_stream;
+    PL_CUDA(h, cudaMemsetAsync(h->S, 0, sizeof(float) * (size_t)h->R * (size_t)h->N, st));
+    PL_CUDA(h, cudaStreamSynchronize(st));
+    h->have_work = false;
+    return PLSPEC_OK;
+}
+
+int plspec_destroy(plspec_handle h) {
+    free_ctx(h);
+    return PLSPEC_OK;
+}
+
+int plspec_get_stats(plspec_handle h, plspec_stats_t *out) {
+    if (!h || !out) return PLSPEC_ERR_INVALID_ARG;
+    *out = h->stats;
+    return PLSPEC_OK;
+}
+
+int plspec_last_cuda_error(plspec_handle h) { return h ? h->last_cuda : 0; }
+
+const char *plspec_strerror(int status) {
+    switch (status) {
+        case PLSPEC_OK: return "ok";
+        case PLSPEC_ERR_INVALID_ARG: return "invalid argument";
+        case PLSPEC_ERR_ALLOC: return "allocation failed";
+        case PLSPEC_ERR_CUDA: return "CUDA call failed (see plspec_last_cuda_error)";
+        case PLSPEC_ERR_UNSUPPORTED: return "unsupported on this device or build";
+    }
+    return "unknown status";
+}
+
+const char *plspec_version(void) { return "plspec 0.1 (sm_100a)"; }
+
+}  // extern "C"

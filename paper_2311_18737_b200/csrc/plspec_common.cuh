@@ -1,0 +1,131 @@
+// plspec_common.cuh -- shared device helpers for the plspec kernels (sm_100a).
+//
+// Notation follows include/plspec.h and the paper: V = received voltages, C = transmit
+// code, d = decoded window, X = its length-N DFT,
+// S[r][f] = accumulated |X|^2 (Eq. 8).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <type_traits>
+
+namespace plspec {
+
+enum { DT_CF32 = 0, DT_SC16 = 1 };
+
+// Kernel arguments (one struct, passed by value).
+struct KParams {
+    const void   *V;        // voltages[n_ipp][v_pitch] (float2 or short2 per sample)
+    const float2 *C;        // codes[n_ipp][L]
+    float        *S;        // S_dev[R][Q][Nk]  (Q = N / Nk outer radix; natural order when Q == 1)
+    const float2 *tw1;      // [32][Nk/32]: exp(-2 pi i f1 n' / Nk)   (fused kernel, pass 1 -> 2)
+    const float2 *twN;      // [N]: exp(-2 pi i e / N), full circle
+    long long     v_pitch;  // samples between successive IPP rows of V
+    int N, Nk, Q, log2Nk;
+    int L;                  // code_len
+    int R, r0, stride;
+    int n_ipp, n_chunks;    // IPPs of this launch are split over n_chunks CTAs per (gate, q)
+    int use_atomic;         // 1: partial sums meet in S via red.global.add.f32
+};
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// (a)(b)
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+// a * conj(b)  -- the decode multiply of PAPER.md:107 ("takes the conjugate of the transmit
+// signal (TX) and complex multiplies that with the corresponding element in the return echo")
+__device__ __forceinline__ float2 cmul_conj(float2 a, float2 b) {
+    return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+
+// Exact int16 -> fp32 for an interleaved (I, Q) pair packed in one 32-bit word, without the
+// quarter-rate I2F pipe: (x ^ 0x8000) is x + 32768 as an unsigned 16-bit value u, and the bit
+// pattern 0x4B000000 | u is the float 2^23 + u, so subtracting 2^23 + 32768 gives x exactly.
+__device__ __forceinline__ float2 sc16_to_f32(uint32_t w) {
+    w ^= 0x80008000u;
+    float re = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)) - 8421376.0f;
+    float im = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)) - 8421376.0f;
+    return make_float2(re, im);
+}
+
+template <int DT>
+__device__ __forceinline__ float2 load_voltage(const void *V, long long idx) {
+    if constexpr (DT == DT_CF32) {
+        return __ldg(reinterpret_cast<const float2 *>(V) + idx);
+    } else {
+        return sc16_to_f32(__ldg(reinterpret_cast<const uint32_t *>(V) + idx));
+    }
+}
+
+// compile-time loop
+template <int B, int E, class F>
+__device__ __forceinline__ void sfor(F &&f) {
+    if constexpr (B < E) {
+        f(std::integral_constant<int, B>{});
+        sfor<B + 1, E>(f);
+    }
+}
+
+template <int LOG>
+__host__ __device__ constexpr int brev(int j) {
+    int r = 0;
+    for (int b = 0; b < LOG; b++) r |= ((j >> b) & 1) << (LOG - 1 - b);
+    return r;
+}
+__host__ __device__ constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
+
+// cos(2 pi k / 32), k = 0..8, correctly rounded to fp32 from float64.
+template <int K> struct Cos32Tab;
+template <> struct Cos32Tab<0> { static constexpr float v = 1.0f; };
+template <> struct Cos32Tab<1> { static constexpr float v = 0.98078528040323044913f; };
+template <> struct Cos32Tab<2> { static constexpr float v = 0.92387953251128675613f; };
+template <> struct Cos32Tab<3> { static constexpr float v = 0.83146961230254523708f; };
+template <> struct Cos32Tab<4> { static constexpr float v = 0.70710678118654752440f; };
+template <> struct Cos32Tab<5> { static constexpr float v = 0.55557023301960222474f; };
+template <> struct Cos32Tab<6> { static constexpr float v = 0.38268343236508977173f; };
+template <> struct Cos32Tab<7> { static constexpr float v = 0.19509032201612826785f; };
+template <> struct Cos32Tab<8> { static constexpr float v = 0.0f; };
+
+template <int K>
+__host__ __device__ constexpr float cos32() {
+    constexpr int k = ((K % 32) + 32) % 32;
+    if constexpr (k > 16) return cos32<32 - k>();
+    else if constexpr (k > 8) return -Cos32Tab<16 - k>::v;
+    else return Cos32Tab<k>::v;
+}
+template <int K>
+__host__ __device__ constexpr float sin32() { return cos32<K + 24>(); }   // sin(x) = cos(x - pi/2)
+
+// d * W_32^K,  W_32 = exp(-2 pi i / 32),  0 <= K < 16
+template <int K>
+__device__ __forceinline__ float2 mul_w32(float2 d) {
+    if constexpr (K == 0) return d;
+    else if constexpr (K == 8) return make_float2(d.y, -d.x);                     // * (-i)
+    else if constexpr (K == 4) { constexpr float c = Cos32Tab<4>::v; return make_float2(c * (d.x + d.y), c * (d.y - d.x)); }
+    else if constexpr (K == 12) { constexpr float c = Cos32Tab<4>::v; return make_float2(c * (d.y - d.x), -c * (d.x + d.y)); }
+    else {
+        constexpr float c = cos32<K>(), s = sin32<K>();                           // W = c - i s
+        return make_float2(d.x * c + d.y * s, d.y * c - d.x * s);
+    }
+}
+
+// In-register radix-2 decimation-in-frequency DFT of R points (R = 2..32, power of two):
+// on return v[j] = X[brev(j)] with X[k] = sum_t v_in[t] exp(-2 pi i k t / R).
+template <int R>
+__device__ __forceinline__ void dft_dif(float2 (&v)[R]) {
+    constexpr int LOG = ilog2(R);
+    sfor<0, LOG>([&](auto s_) {
+        constexpr int half = R >> (decltype(s_)::value + 1);
+        sfor<0, R / 2>([&](auto b_) {
+            constexpr int b = decltype(b_)::value;
+            constexpr int k = b % half;
+            constexpr int i = (b / half) * 2 * half + k;
+            float2 a = v[i], c = v[i + half];
+            v[i] = cadd(a, c);
+            v[i + half] = mul_w32<k * (16 / half)>(csub(a, c));   // W_{2 half}^k
+        });
+    });
+}
+
+}  // namespace plspec

@@ -1,0 +1,62 @@
+"""CPU-side checks of the boundary: libplspec.so builds, loads and exports every symbol that
+include/plspec.h declares; status strings; graceful failure without a device.  No compute."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2311_18737_b200 import binding as pl
+from paper_2311_18737_b200 import build as plbuild
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "plspec.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(plspec_[a-z_]+)\s*\(", src)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    plbuild.build()
+    return pl.lib()
+
+
+def test_header_and_binding_agree():
+    assert declared_functions() == sorted(pl.EXPORTED_SYMBOLS)
+
+
+def test_library_exports_every_declared_symbol(lib):
+    raw = ctypes.CDLL(pl.LIB_PATH)
+    for name in declared_functions():
+        assert hasattr(raw, name), f"libplspec.so does not export {name}"
+
+
+def test_strerror_and_version(lib):
+    assert pl.strerror(pl.PLSPEC_OK) == "ok"
+    for code in (pl.PLSPEC_ERR_INVALID_ARG, pl.PLSPEC_ERR_ALLOC, pl.PLSPEC_ERR_CUDA, pl.PLSPEC_ERR_UNSUPPORTED, -99):
+        assert isinstance(pl.strerror(code), str) and pl.strerror(code)
+    assert "plspec" in pl.plspec_version()
+
+
+def test_no_silent_cpu_fallback(lib):
+    """Without a CUDA device create must fail with an error code -- never compute on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    h = ctypes.c_void_p(123)
+    rc = lib.plspec_create(1024, 1024, 4, 0, 1, 0, 0, ctypes.byref(h))
+    assert rc in (pl.PLSPEC_ERR_CUDA, pl.PLSPEC_ERR_UNSUPPORTED) and not h.value
+    rc = lib.plspec_create(1000, 1024, 4, 0, 1, 0, 0, ctypes.byref(h))
+    assert rc == pl.PLSPEC_ERR_INVALID_ARG          # argument checks come first, device or not
+    assert lib.plspec_accumulate(None, None, None, 1, None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_finalize(None, None) == pl.PLSPEC_ERR_INVALID_ARG
+
+
+def test_binding_has_no_compute():
+    """The binding marshals arguments only: no numpy/torch arithmetic on data inside it."""
+    src = open(os.path.join(ROOT, "paper_2311_18737_b200", "binding.py")).read()
+    for banned in ("np.fft", "torch.fft", "np.abs", "np.conj", "oracle"):
+        assert banned not in src.split('"""', 2)[2], banned

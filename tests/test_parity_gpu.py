@@ -1,0 +1,234 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by
+element on the same seeded inputs.  Bar (BASELINE.json north_star):
+
+    max_f |S_gpu[r][f] - S_ref[r][f]| / mean_f(S_ref[r][f]) <= 1e-4   for every range gate r,
+
+and S_gpu == 0 exactly where the input is zero.  Run on the B200 box: pytest -m gpu.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2311_18737_b200 import synth
+from paper_2311_18737_b200 import binding as pl
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+rng = np.random.default_rng(7)
+
+
+def gate_metric(S_gpu, S_ref):
+    S_gpu = np.asarray(S_gpu, dtype=np.float64)
+    mean = S_ref.mean(axis=1)
+    assert np.all(mean > 0)
+    return np.abs(S_gpu - S_ref).max(axis=1) / mean
+
+
+def to_dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(w, V, C, *, kernel=pl.KERNEL_AUTO, chunks=0, splits=(None,), where="device", batch=0):
+    """One integration through the C ABI; returns S as float32 numpy [R][N]."""
+    S = torch.full((w.n_ranges, w.N), -1.0, dtype=torch.float32, device="cuda")
+    with pl.Integrator.for_workload(w, kernel=kernel, ipp_chunks=chunks, h2d_batch=batch) as it:
+        bounds = [0] + [s for s in splits if s is not None] + [w.n_ipp]
+        keep = []
+        for a, b in zip(bounds[:-1], bounds[1:]):
+            if where == "device":
+                v, c = to_dev(V[a:b]), to_dev(C[a:b])
+            elif where == "pinned":
+                v = torch.from_numpy(np.ascontiguousarray(V[a:b])).pin_memory()
+                c = torch.from_numpy(np.ascontiguousarray(C[a:b])).pin_memory()
+            else:                                   # pageable numpy
+                v, c = np.ascontiguousarray(V[a:b]), np.ascontiguousarray(C[a:b])
+            keep.append((v, c))
+            it.accumulate(v, c, b - a)
+        it.finalize(S)
+        stats = it.stats()
+    return S.cpu().numpy(), stats
+
+
+def check(w, V, C, **kw):
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    S_gpu, stats = run_gpu(w, V, C, **kw)
+    m = gate_metric(S_gpu, S_ref)
+    assert m.max() <= TOL, f"{w.name}: worst gate metric {m.max():.3e} at gate {int(m.argmax())}"
+    return S_gpu, S_ref, stats
+
+
+def random_case(N, L, R, r0, stride, P, dtype, pad=3, complex_code=True):
+    M = r0 + (R - 1) * stride + L + pad
+    w = synth.Workload(f"rand N={N}", N, L, R, r0, stride, M, P, dtype, "x", "x")
+    if complex_code:
+        C = np.exp(2j * np.pi * rng.random((P, L))).astype(np.complex64) * \
+            (0.5 + rng.random((P, L))).astype(np.float32)
+    else:
+        C = (2.0 * rng.integers(0, 2, size=(P, L)) - 1.0).astype(np.complex64)
+    if dtype == synth.CF32:
+        V = (rng.standard_normal((P, M)) + 1j * rng.standard_normal((P, M))).astype(np.complex64)
+    else:
+        V = rng.integers(-3000, 3000, size=(P, M, 2)).astype(np.int16)
+        V[0, 0] = (-32768, 32767)
+    return w, V, C
+
+
+# ---- BASELINE configs --------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", [pl.KERNEL_FUSED, pl.KERNEL_GENERIC])
+def test_cfg1_full(kernel):
+    w = synth.CONFIGS["cfg1"]
+    V, C = synth.make_inputs(w)
+    S_gpu, S_ref, stats = check(w, V, C, kernel=kernel)
+    assert stats["kernel_kind"] == kernel and stats["kernel_launches"] >= 1
+    r, f = np.unravel_index(np.argmax(S_gpu), S_gpu.shape)
+    assert (r, f) == (20, 100)                       # the injected tone: gate 20, bin 100
+
+
+def test_cfg2_scaled_ragged():
+    w = synth.scaled(synth.CONFIGS["cfg2"], n_ranges=37, n_ipp=7)
+    V, C = synth.make_inputs(w)
+    check(w, V, C)
+    check(w, V, C, chunks=3)                         # partial sums meet through atomics
+
+
+def test_cfg3_scaled_sc16():
+    w = synth.scaled(synth.CONFIGS["cfg3"], n_ranges=13, n_ipp=5)
+    V, C = synth.make_inputs(w)
+    assert V.dtype == np.int16
+    check(w, V, C)
+
+
+def test_cfg4_scaled_chirp_n65536():
+    w = synth.scaled(synth.CONFIGS["cfg4"], n_ranges=5, n_ipp=3)
+    V, C = synth.make_inputs(w)
+    assert np.abs(C.imag).max() > 0.5                # complex code: pins conj(code) (reading A4)
+    check(w, V, C)
+
+
+def test_cfg5_scaled_stream_from_pinned_host():
+    w = synth.scaled(synth.CONFIGS["cfg5"], n_ranges=21, n_ipp=9, ipp_len=30000)
+    V, C = synth.make_inputs(w)
+    _, _, stats = check(w, V, C, where="pinned", batch=2)
+    esz = 4
+    assert stats["h2d_bytes"] == w.n_ipp * (w.span * esz + w.code_len * 8)   # span only, not whole IPPs
+    assert stats["kernel_launches"] == 5
+
+
+# ---- every FFT length, both kernels, awkward geometry --------------------------------------------
+@pytest.mark.parametrize("N", [16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384, 32768, 65536])
+def test_all_lengths_generic(N):
+    R = 5 if N <= 4096 else 2
+    w, V, C = random_case(N, N - N // 4 + 1, R, 2, 3, 3, synth.CF32)
+    check(w, V, C, kernel=pl.KERNEL_GENERIC)
+
+
+@pytest.mark.parametrize("N", [1024, 2048, 4096, 8192, 16384, 32768, 65536])
+@pytest.mark.parametrize("dtype", [synth.CF32, synth.SC16])
+def test_all_lengths_fused(N, dtype):
+    R = 6 if N <= 4096 else 3
+    w, V, C = random_case(N, N - 5, R, 1, 7, 3, dtype)
+    S_gpu, S_ref, _ = check(w, V, C, kernel=pl.KERNEL_FUSED)
+    # and the two GPU implementations agree with each other
+    S_gen, _ = run_gpu(w, V, C, kernel=pl.KERNEL_GENERIC)
+    assert gate_metric(S_gen, S_ref).max() <= TOL
+
+
+def test_short_code_zero_padding():
+    w, V, C = random_case(4096, 1000, 4, 0, 1, 2, synth.CF32)
+    check(w, V, C)
+
+
+# ---- accumulation semantics ------------------------------------------------------------------------
+def test_split_calls_host_and_device_and_finalize_zeroes():
+    w, V, C = random_case(2048, 2048, 9, 3, 2, 6, synth.CF32, complex_code=False)
+    S1, S_ref, _ = check(w, V, C)
+    S2, _ = run_gpu(w, V, C, splits=(1, 4))
+    S3, _ = run_gpu(w, V, C, where="pageable", splits=(2,))
+    for S in (S2, S3):
+        assert gate_metric(S, S_ref).max() <= TOL
+    with pl.Integrator.for_workload(w) as it:
+        out = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+        it.accumulate(to_dev(V), to_dev(C))
+        it.finalize(out)
+        it.finalize(out)                                  # nothing accumulated since: all zeros
+        assert float(out.abs().max()) == 0.0
+        it.accumulate(to_dev(V), to_dev(C))
+        it.reset()
+        it.accumulate(to_dev(V[:2]), to_dev(C[:2]))
+        host_out = np.empty((w.n_ranges, w.N), dtype=np.float32)
+        it.finalize(host_out)                             # host S_out
+    ref2 = oracle.spectra(V[:2], C[:2], N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    assert gate_metric(host_out, ref2).max() <= TOL
+
+
+def test_zero_input_gives_exact_zero():
+    w, V, C = random_case(1024, 1024, 4, 0, 1, 2, synth.SC16)
+    V[:] = 0
+    S, _ = run_gpu(w, V, C)
+    assert np.all(S == 0.0)
+
+
+def test_user_stream():
+    w, V, C = random_case(1024, 1024, 8, 0, 1, 4, synth.CF32)
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges)
+    st = torch.cuda.Stream()
+    out = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+    v, c = to_dev(V), to_dev(C)
+    torch.cuda.synchronize()
+    with pl.Integrator.for_workload(w) as it:
+        it.accumulate(v[:2], c[:2], 2, stream=st)
+        it.accumulate(v[2:], c[2:], 2)                    # default stream: must order after `st`
+        it.finalize(out)
+    assert gate_metric(out.cpu().numpy(), S_ref).max() <= TOL
+
+
+# ---- argument errors --------------------------------------------------------------------------------
+def test_argument_errors():
+    bad = [
+        dict(N=1000), dict(N=8), dict(N=131072), dict(code_len=0), dict(code_len=2049),
+        dict(n_ranges=0), dict(stride=0), dict(r0=-1), dict(dtype=7), dict(ipp_len=100),
+    ]
+    base = dict(N=2048, code_len=2048, n_ranges=4, r0=0, stride=1, ipp_len=0, dtype=0)
+    for b in bad:
+        args = {**base, **b}
+        with pytest.raises(pl.PlspecError) as e:
+            pl.plspec_create(*args.values())
+        assert e.value.status == pl.PLSPEC_ERR_INVALID_ARG
+    h = pl.plspec_create(*base.values())
+    try:
+        v = torch.zeros((1, 2051), dtype=torch.complex64, device="cuda")
+        c = torch.ones((1, 2048), dtype=torch.complex64, device="cuda")
+        pl.plspec_accumulate(h, v, c, 0)                  # n_ipp == 0: successful no-op
+        with pytest.raises(pl.PlspecError):
+            pl.plspec_accumulate(h, v, c, -1)
+        with pytest.raises(pl.PlspecError):
+            pl.plspec_accumulate(h, None, c, 1)
+        with pytest.raises(pl.PlspecError):               # mixed host / device pointers
+            pl.plspec_accumulate(h, v, np.ones((1, 2048), dtype=np.complex64), 1)
+        with pytest.raises(pl.PlspecError):
+            pl.plspec_finalize(h, None)
+        with pytest.raises(pl.PlspecError):
+            pl.plspec_configure(h, 99, 1)
+    finally:
+        pl.plspec_destroy(h)
+    assert pl.lib().plspec_destroy(None) == 0
+
+
+# ---- full size, in the launch configuration bench.py times; oracle on sampled gates --------------------
+def test_cfg3_full_size_sampled_gates():
+    w = synth.CONFIGS["cfg3"]
+    V, C = synth.make_inputs(w)
+    S_gpu, stats = run_gpu(w, V, C)
+    gates = [0, 1, 147, 148, 500, 998, 999]
+    for g in gates:
+        ref = oracle.spectra(V, C, N=w.N, n_ranges=1, r0=w.r0 + g * w.stride, stride=1)
+        m = gate_metric(S_gpu[g:g + 1], ref)
+        assert m.max() <= TOL, f"gate {g}: {m.max():.3e}"
+    # properties that hold at any size: Parseval per gate (sum_f S = N * window energy, |code| = 1)
+    Vf = V[..., 0].astype(np.float64) ** 2 + V[..., 1].astype(np.float64) ** 2
+    cs = np.concatenate([np.zeros((w.n_ipp, 1)), np.cumsum(Vf, axis=1)], axis=1)
+    for g in range(0, w.n_ranges, 37):
+        energy = (cs[:, g + w.code_len] - cs[:, g]).sum()
+        assert abs(S_gpu[g].astype(np.float64).sum() / (w.N * energy) - 1.0) < 1e-5
