@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py -- decoded range-gate spectra/s of the plspec hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+    (N > 1: python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...)
+
+A "step" is one whole integration of the workload: plspec_accumulate over all its IPPs (sc16
+conversion, decode, FFT, |X|^2, accumulation -- every row of SURVEY.md 8(a)) followed by
+plspec_finalize (spectra written out once, accumulators cleared).  Default workload: cfg3 =
+BASELINE.json configs[2] (N = 16384, the length the metric is quoted at).
+
+value  : spectra/s with inputs resident in HBM, timed on the device with CUDA events,
+         L2 flushed between steps, max over ranks.
+e2e    : the same metric through the same C-ABI calls with HOST (pinned) buffers: the H2D copy
+         of voltages + codes and the D2H copy of S are inside the timed region.
+roofline: the fused kernel against the FP32 ALU roofline (5 N log2 N flops per window).
+cpu_baseline: the float64 oracle on this box's host cores, on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2311_18737_b200 import synth  # noqa: E402
+
+METRIC = "decoded range-gate spectra/s at N=16384"
+UNIT = "spectra/s"
+# FP32 ALU peak: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz max SM clock (B200_PROFILING.md
+# unit counts and clocks).  Measured FFMA issue rate on this pool: 124.6 of 128.
+N_SM, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
+ALU_PEAK_TFLOPS = N_SM * FP32_LANES * 2 * SM_MAX_GHZ / 1e3
+PAPER_BEST_SPECTRA_PER_S = 409600 / 1.488      # GTX 780 Ti, PAPER.md:139 (workload "paper" only)
+
+
+def metric_name(w):
+    return METRIC if w.N == 16384 else f"decoded range-gate spectra/s at N={w.N}"
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+def cpu_oracle_sample(w, V, C, target_s=12.0, steps=1):
+    """Time the oracle as it stands on a bounded sample: a subset of gates over ALL IPPs
+    (gates are independent and cost the same, so the rate extrapolates exactly)."""
+    import oracle
+    cores = oracle.max_threads()
+    # calibrate with all threads busy: `cores` gates x a few IPPs
+    pc = min(4, w.n_ipp)
+    t0 = time.perf_counter()
+    oracle.spectra(V[:pc], C[:pc], N=w.N, n_ranges=min(cores, w.n_ranges), r0=w.r0, stride=w.stride)
+    per_round = (time.perf_counter() - t0) / pc * w.n_ipp        # seconds for `cores` gates x all IPPs
+    rounds = int(max(1, target_s / max(per_round, 1e-9)))
+    gates = min(w.n_ranges, rounds * cores)
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        oracle.spectra(V, C, N=w.N, n_ranges=gates, r0=w.r0, stride=w.stride)
+        times.append(time.perf_counter() - t0)
+    dt = float(np.mean(times))
+    return {"value": gates * w.n_ipp / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{gates} of {w.n_ranges} gates x all {w.n_ipp} IPPs of {w.name} "
+                      f"({gates * w.n_ipp} windows, {dt:.1f} s per step, float64 radix-2, OpenMP over gates)"}, dt
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle (the only 'reference implementation' this tier has)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    V, C = synth.make_inputs(w)
+    for _ in range(min(args.warmup, 1)):
+        cpu_oracle_sample(w, V, C, target_s=2.0)
+    cb, dt = cpu_oracle_sample(w, V, C, target_s=10.0, steps=max(1, min(args.steps, 5)))
+    line = {
+        "impl": "reference", "metric": metric_name(w), "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "N": w.N, "n_ranges": w.n_ranges, "n_ipp": w.n_ipp,
+                   "note": "each step is a bounded sample of the workload (subset of gates, all IPPs)"},
+        "cpu_baseline": cb,
+        "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg3", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 fused")
+    ap.add_argument("--chunks", type=int, default=0)
+    args = ap.parse_args()
+    w = synth.CONFIGS[args.workload]
+    if args.impl == "reference":
+        return run_reference(args, w)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    from paper_2311_18737_b200 import binding as pl
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the plspec path has no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- inputs: every rank integrates its own batch of the same shape (weak scaling, no
+    # data-path collective: integrations are independent problems).
+    wr = synth.Workload(**{**w.__dict__, "seed": w.seed + 17 * rank})
+    V_np, C_np = synth.make_inputs(wr, full_ranges=w.n_ranges)
+    V_pin = torch.from_numpy(V_np).pin_memory()
+    C_pin = torch.from_numpy(C_np).pin_memory()
+    V_dev, C_dev = V_pin.cuda(), C_pin.cuda()
+    S_dev = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+    S_pin = torch.empty((w.n_ranges, w.N), dtype=torch.float32).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    it = pl.Integrator.for_workload(w, kernel=args.kernel, ipp_chunks=args.chunks)
+
+    def step_device(ev=None):
+        if ev:
+            ev[0].record()
+        it.accumulate(V_dev, C_dev, w.n_ipp)
+        if ev:
+            ev[1].record()
+        it.finalize(S_dev)
+
+    def step_host():
+        it.accumulate(V_pin, C_pin, w.n_ipp)
+        it.finalize(S_pin)
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        flush.fill_(1)
+        step_device()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = it.stats()["kernel_launches"]
+    step_ms, kern_ms = [], []
+    t_wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        flush.fill_(2)                                              # L2 flush, outside the event pair
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step_device((k0, k1))
+        e1.record()
+        e1.synchronize()
+        step_ms.append(e0.elapsed_time(e1))
+        kern_ms.append(k0.elapsed_time(k1))
+    barrier()
+    wall_s = time.perf_counter() - t_wall0
+    launches = it.stats()["kernel_launches"] - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = float(np.sum(step_ms))
+    stats = it.stats()
+
+    # ---- end to end: host pinned inputs -> S on the host
+    e2e_ms = None
+    if not args.no_e2e:
+        for _ in range(2):
+            step_host()
+        barrier()
+        ts = []
+        for _ in range(args.steps):
+            flush.fill_(3)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            step_host()                                             # finalize blocks until S_pin is complete
+            ts.append((time.perf_counter() - t0) * 1e3)
+        e2e_ms = float(np.sum(ts))
+        barrier()
+
+    # ---- max over ranks
+    if dist is not None:
+        t = torch.tensor([total_ms, e2e_ms or 0.0, float(np.mean(kern_ms))], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_max, kern_mean = [float(x) for x in t.cpu()]
+        e2e_ms = e2e_max if e2e_ms is not None else None
+    else:
+        kern_mean = float(np.mean(kern_ms))
+
+    if rank == 0:
+        windows_per_step = w.windows * world
+        value = windows_per_step * args.steps / (total_ms * 1e-3)
+        esz = 4 if w.dtype == synth.SC16 else 8
+        h2d = w.n_ipp * (w.span * esz + w.code_len * 8)
+        flops_per_launch = w.fft_flops                              # 5 N log2 N x windows of one launch
+        achieved = flops_per_launch / (kern_mean * 1e-3) / 1e12
+        traffic = None
+        tfile = os.path.join(ROOT, "profiles", "traffic_bytes.json")
+        if os.path.exists(tfile):
+            try:
+                traffic = json.load(open(tfile)).get(w.name)
+            except Exception:
+                traffic = None
+        line = {
+            "metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak",
+            "vs_baseline": (value / PAPER_BEST_SPECTRA_PER_S) if w.name == "paper" else None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "code_len": w.code_len, "n_ranges": w.n_ranges,
+                       "stride": w.stride, "n_ipp": w.n_ipp, "ipp_len": w.ipp_len,
+                       "input": "sc16" if w.dtype == synth.SC16 else "complex64",
+                       "windows_per_step": w.windows, "l2": "flushed between steps (256 MB write)",
+                       "parallelism": f"{world} independent integrations (one per GPU)",
+                       "kernel": {1: "generic", 2: "fused"}[stats["kernel_kind"]],
+                       "ipp_chunks": stats["ipp_chunks_last"]},
+            "realtime_factor": w.data_seconds * world * args.steps / (total_ms * 1e-3),
+            "wall_s_timed_region": wall_s,
+            "clocks": clocks,
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                         "frac": achieved / ALU_PEAK_TFLOPS, "traffic": traffic,
+                         "kernel": "fused_kernel" if stats["kernel_kind"] == 2 else "generic_kernel",
+                         "kernel_ms": kern_mean, "flops_per_launch": flops_per_launch,
+                         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); "
+                                        "MEASURED_PEAKS.json holds no FP32 ALU figure",
+                         "hbm_bytes_algorithmic": w.n_ipp * (w.ipp_len * esz + w.code_len * 8) + w.n_ranges * w.N * 4},
+        }
+        if e2e_ms is not None:
+            line["e2e"] = {"value": windows_per_step * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+                           "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(w.n_ranges * w.N * 4),
+                           "ms_per_step": e2e_ms / args.steps,
+                           "realtime_factor": w.data_seconds * world * args.steps / (e2e_ms * 1e-3)}
+        if world == 1 and not args.no_cpu_baseline:
+            cb, _ = cpu_oracle_sample(w, V_np, C_np)
+            line["cpu_baseline"] = cb
+        print(json.dumps(line), flush=True)
+    it.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
