@@ -3,6 +3,7 @@
 // step of decode / FFT / power / accumulate runs in the kernels of plspec_kernels.cuh.
 #include "../../include/plspec.h"
 #include "plspec_kernels.cuh"
+#include "plspec_fused.cuh"
 
 #include <cmath>
 #include <cstdlib>
@@ -33,7 +34,8 @@ struct plspec_ctx {
     int device = 0, n_sm = 0;
     // kernel selection
     int kind = 2;                    // 1 generic, 2 fused
-    int Nk = 0, Q = 1, R3 = 1;
+    int Nk = 0, Q = 1, RA = 1;   // N = Q * Nk, Nk = 1024 * RA (fused)
+    int gates_per_cta = 1, n_groups = 0;
     int opt_kernel = 0, opt_chunks = 0, opt_batch = 0;
     int block = 0;
     size_t smem = 0;
@@ -41,8 +43,8 @@ struct plspec_ctx {
     const void *kfunc = nullptr;
     // device state
     float  *S = nullptr;             // [R][Q][Nk]
-    float  *S_tmp = nullptr;         // interleave target when S_out is a host pointer and Q > 1
-    float2 *tw1 = nullptr, *twN = nullptr;
+    float  *S_tmp = nullptr;         // un-permute target when S_out is a host pointer
+    float2 *twA = nullptr, *twB = nullptr, *twN = nullptr;
     // host pipeline
     cudaStream_t copy_stream = nullptr;
     Slot slot[kSlots];
@@ -71,44 +73,26 @@ namespace {
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
-template <int R3, int Q>
+template <int RA, int Q>
 const void *fused_ptr(int dt) {
-    return dt == DT_CF32 ? (const void *)fused_kernel<R3, Q, DT_CF32>
-                         : (const void *)fused_kernel<R3, Q, DT_SC16>;
+    return dt == DT_CF32 ? (const void *)fused_kernel<RA, Q, DT_CF32>
+                         : (const void *)fused_kernel<RA, Q, DT_SC16>;
 }
-// the outer radix Q > 1 only occurs with the largest inner size (Nk = 16384, R3 = 16)
-const void *fused_lookup(int R3, int Q, int dt) {
+// the outer radix Q > 1 only occurs with the largest inner size (Nk = 16384, RA = 16)
+const void *fused_lookup(int RA, int Q, int dt) {
     if (Q == 1) {
-        switch (R3) {
+        switch (RA) {
             case 1:  return fused_ptr<1, 1>(dt);
             case 2:  return fused_ptr<2, 1>(dt);
             case 4:  return fused_ptr<4, 1>(dt);
             case 8:  return fused_ptr<8, 1>(dt);
             case 16: return fused_ptr<16, 1>(dt);
         }
-    } else if (R3 == 16) {
+    } else if (RA == 16) {
         if (Q == 2) return fused_ptr<16, 2>(dt);
         if (Q == 4) return fused_ptr<16, 4>(dt);
     }
     return nullptr;
-}
-
-bool g_tw2_ready[64] = {false};
-
-int upload_tw2(plspec_ctx *h) {
-    if (h->device < 64 && g_tw2_ready[h->device]) return PLSPEC_OK;
-    std::vector<float2> t(960);
-    for (int R3 = 2; R3 <= 16; R3 *= 2) {
-        const int M1 = 32 * R3;
-        for (int t3 = 0; t3 < R3; t3++)
-            for (int f2 = 0; f2 < 32; f2++) {
-                double a = -2.0 * M_PI * (double)((t3 * f2) % M1) / (double)M1;
-                t[tw2_offset(R3) + t3 * 32 + f2] = make_float2((float)cos(a), (float)sin(a));
-            }
-    }
-    PL_CUDA(h, cudaMemcpyToSymbol(c_tw2, t.data(), sizeof(float2) * 960));
-    if (h->device < 64) g_tw2_ready[h->device] = true;
-    return PLSPEC_OK;
 }
 
 // Resolve kernel kind / geometry from N and the options; (re)build what depends on it.
@@ -120,12 +104,14 @@ int select_kernel(plspec_ctx *h) {
     h->Q = h->N / h->Nk;
     const int dt = h->dtype == PLSPEC_SC16 ? DT_SC16 : DT_CF32;
     if (kind == 2) {
-        h->R3 = h->Nk / 1024;
-        h->block = 32 * h->R3;
-        h->smem = (size_t)h->block * 33 * sizeof(float2);
-        h->kfunc = fused_lookup(h->R3, h->Q, dt);
+        h->RA = h->Nk / 1024;
+        h->gates_per_cta = 16 / h->RA;
+        h->block = kFusedThreads;
+        h->smem = (size_t)kFusedSmemBytes;
+        h->kfunc = fused_lookup(h->RA, h->Q, dt);
     } else {
-        h->R3 = 0;
+        h->RA = 0;
+        h->gates_per_cta = 1;
         h->block = h->Nk / 2 < 32 ? 32 : (h->Nk / 2 > 512 ? 512 : h->Nk / 2);
         h->smem = (size_t)h->Nk * (sizeof(float2) + sizeof(float));
         h->kfunc = dt == DT_CF32 ? (const void *)generic_kernel<DT_CF32> : (const void *)generic_kernel<DT_SC16>;
@@ -136,6 +122,7 @@ int select_kernel(plspec_ctx *h) {
     PL_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->kfunc, h->block, h->smem));
     if (occ < 1) return PLSPEC_ERR_UNSUPPORTED;
     h->slots_per_wave = occ * h->n_sm;
+    h->n_groups = (h->R + h->gates_per_cta - 1) / h->gates_per_cta;
     h->stats.kernel_kind = kind;
     return PLSPEC_OK;
 }
@@ -143,7 +130,7 @@ int select_kernel(plspec_ctx *h) {
 // IPP chunks per (gate, q): more CTAs than one wave can hold, whole waves, few flushes.
 int pick_chunks(const plspec_ctx *h, int n_ipp) {
     if (h->opt_chunks > 0) return h->opt_chunks < n_ipp ? h->opt_chunks : n_ipp;
-    const long long base = (long long)h->R * h->Q;
+    const long long base = (long long)h->n_groups * h->Q;
     const int slots = h->slots_per_wave;
     int best = 1;
     double best_score = -1.0;
@@ -161,15 +148,16 @@ int pick_chunks(const plspec_ctx *h, int n_ipp) {
 int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0,
                       int n_ipp, cudaStream_t stream) {
     KParams P;
-    P.V = dV; P.C = dC; P.S = h->S; P.tw1 = h->tw1; P.twN = h->twN;
+    P.V = dV; P.C = dC; P.S = h->S; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
     P.v_pitch = v_pitch;
     P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
     P.L = h->L; P.R = h->R; P.r0 = r0; P.stride = h->stride;
+    P.n_groups = h->n_groups;
     P.n_ipp = n_ipp;
     P.n_chunks = pick_chunks(h, n_ipp);
     P.use_atomic = P.n_chunks > 1 ? 1 : 0;
     h->stats.ipp_chunks_last = P.n_chunks;
-    const long long tiles = (long long)h->R * h->Q * P.n_chunks;
+    const long long tiles = (long long)h->n_groups * h->Q * P.n_chunks;
     if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
     void *args[] = {&P};
     PL_CUDA(h, cudaLaunchKernel(h->kfunc, dim3((unsigned)tiles), dim3((unsigned)h->block), args, h->smem, stream));
@@ -253,20 +241,39 @@ int build_tables(plspec_ctx *h) {
     }
     PL_CUDA(h, cudaMalloc((void **)&h->twN, sizeof(float2) * (size_t)h->N));
     PL_CUDA(h, cudaMemcpy(h->twN, t.data(), sizeof(float2) * (size_t)h->N, cudaMemcpyHostToDevice));
-    // pass-1 -> pass-2 twiddles of the fused kernel: [f1][n'] = W_Nk^{f1 n'}
+    // fused kernel tables (plspec_fused.cuh), every entry rounded once from float64
     const int Nk = h->N < kMaxNk ? h->N : kMaxNk;
     if (Nk >= 1024) {
-        const int M1 = Nk / 32;
+        const int RA = Nk / 1024;
+        // pass A -> B1: W_Nk^{t_lo f_hi}, t_lo = 64 a' + lane + 32 o, packed over o: [a'][f_hi][re/im][lane]
         std::vector<float2> u((size_t)Nk);
-        for (int f1 = 0; f1 < 32; f1++)
-            for (int n = 0; n < M1; n++) {
-                double a = -2.0 * M_PI * (double)(((long long)f1 * n) % Nk) / (double)Nk;
-                u[(size_t)f1 * M1 + n] = make_float2((float)cos(a), (float)sin(a));
+        for (int ap = 0; ap < 16; ap++)
+            for (int f = 0; f < RA; f++)
+                for (int lane = 0; lane < 32; lane++) {
+                    double w[2][2];
+                    for (int o = 0; o < 2; o++) {
+                        const long long t_lo = 64 * ap + lane + 32 * o;
+                        const double a = -2.0 * M_PI * (double)((t_lo * f) % Nk) / (double)Nk;
+                        w[o][0] = cos(a); w[o][1] = sin(a);
+                    }
+                    for (int k = 0; k < 2; k++)
+                        u[(size_t)((ap * RA + f) * 2 + k) * 32 + lane] = make_float2((float)w[0][k], (float)w[1][k]);
+                }
+        PL_CUDA(h, cudaMalloc((void **)&h->twA, sizeof(float2) * (size_t)Nk));
+        PL_CUDA(h, cudaMemcpy(h->twA, u.data(), sizeof(float2) * (size_t)Nk, cudaMemcpyHostToDevice));
+        // pass B1 -> B2: W_1024^{b c}, packed over (c', c' + 16): [c'][re/im][b]
+        std::vector<float2> v(1024);
+        for (int c = 0; c < 16; c++)
+            for (int b = 0; b < 32; b++) {
+                const double a0 = -2.0 * M_PI * (double)((b * c) % 1024) / 1024.0;
+                const double a1 = -2.0 * M_PI * (double)((b * (c + 16)) % 1024) / 1024.0;
+                v[(size_t)(c * 2 + 0) * 32 + b] = make_float2((float)cos(a0), (float)cos(a1));
+                v[(size_t)(c * 2 + 1) * 32 + b] = make_float2((float)sin(a0), (float)sin(a1));
             }
-        PL_CUDA(h, cudaMalloc((void **)&h->tw1, sizeof(float2) * (size_t)Nk));
-        PL_CUDA(h, cudaMemcpy(h->tw1, u.data(), sizeof(float2) * (size_t)Nk, cudaMemcpyHostToDevice));
+        PL_CUDA(h, cudaMalloc((void **)&h->twB, sizeof(float2) * 1024));
+        PL_CUDA(h, cudaMemcpy(h->twB, v.data(), sizeof(float2) * 1024, cudaMemcpyHostToDevice));
     }
-    return upload_tw2(h);
+    return PLSPEC_OK;
 }
 
 void free_ctx(plspec_ctx *h) {
@@ -280,7 +287,8 @@ void free_ctx(plspec_ctx *h) {
     }
     if (h->S) cudaFree(h->S);
     if (h->S_tmp) cudaFree(h->S_tmp);
-    if (h->tw1) cudaFree(h->tw1);
+    if (h->twA) cudaFree(h->twA);
+    if (h->twB) cudaFree(h->twB);
     if (h->twN) cudaFree(h->twN);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     if (h->work_done) cudaEventDestroy(h->work_done);
@@ -348,6 +356,7 @@ int plspec_configure(plspec_handle h, int option, int value) {
     switch (option) {
         case PLSPEC_OPT_KERNEL: {
             if (value > 2) return PLSPEC_ERR_INVALID_ARG;
+            if (h->have_work) return PLSPEC_ERR_INVALID_ARG;   // the two kernels lay S_dev out differently
             const int old = h->opt_kernel;
             h->opt_kernel = value;
             int rc = select_kernel(h);
@@ -384,7 +393,7 @@ int plspec_finalize(plspec_handle h, float *S_out) {
     cudaStream_t st = h->last_stream;
     const size_t total = (size_t)h->R * (size_t)h->N;
     const float *src = h->S;
-    if (h->Q > 1) {
+    if (h->Q > 1 || h->kind == 2) {                      // S_dev is not in natural bin order
         float *dst = S_out;
         if (!out_dev) {
             if (!h->S_tmp && cudaMalloc((void **)&h->S_tmp, total * sizeof(float)) != cudaSuccess) {
@@ -393,7 +402,8 @@ int plspec_finalize(plspec_handle h, float *S_out) {
             }
             dst = h->S_tmp;
         }
-        interleave_kernel<<<h->n_sm * 8, 256, 0, st>>>(h->S, dst, h->Q, h->Nk, (long long)total);
+        unpermute_kernel<<<h->n_sm * 8, 256, 0, st>>>(h->S, dst, h->Q, h->Nk, h->kind == 2 ? h->RA : 0,
+                                                       (long long)total);
         PL_CUDA(h, cudaGetLastError());
         h->stats.kernel_launches++;
         src = dst;

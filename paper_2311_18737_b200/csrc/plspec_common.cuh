@@ -17,12 +17,14 @@ struct KParams {
     const void   *V;        // voltages[n_ipp][v_pitch] (float2 or short2 per sample)
     const float2 *C;        // codes[n_ipp][L]
     float        *S;        // S_dev[R][Q][Nk]  (Q = N / Nk outer radix; natural order when Q == 1)
-    const float2 *tw1;      // [32][Nk/32]: exp(-2 pi i f1 n' / Nk)   (fused kernel, pass 1 -> 2)
+    const float2 *twA;      // fused kernel, pass A -> B1: [a'][f_hi][re/im][lane] pairs W_Nk^{t_lo f_hi}
+    const float2 *twB;      // fused kernel, pass B1 -> B2: [c'][re/im][lane] pairs W_1024^{b c}
     const float2 *twN;      // [N]: exp(-2 pi i e / N), full circle
     long long     v_pitch;  // samples between successive IPP rows of V
     int N, Nk, Q, log2Nk;
     int L;                  // code_len
     int R, r0, stride;
+    int n_groups;           // gate groups per launch: ceil(R / gates per CTA)
     int n_ipp, n_chunks;    // IPPs of this launch are split over n_chunks CTAs per (gate, q)
     int use_atomic;         // 1: partial sums meet in S via red.global.add.f32
 };

@@ -1,0 +1,322 @@
+// plspec_fused.cuh -- the fused decode + FFT + |X|^2 + accumulate kernel.
+//
+// One CTA = 16 warps = 16 warp-local 1024-point FFTs.  Nk = 1024 * RA (RA = 1, 2, 4, 8, 16) is the
+// length one CTA transforms per window, so a CTA works on G = 16 / RA range gates at a time; N = Q * Nk
+// with an outer radix Q = 1, 2, 4 folded into the load (decimation in frequency, as in the header of
+// plspec_kernels.cuh).  The S accumulators of the CTA's gates stay in registers across all IPPs of
+// the tile and reach HBM once, at the end (PAPER.md:115 accumulates per pulse in device memory).
+//
+// Index algebra (forward DFT, W_n = exp(-2 pi i / n); d = decoded window):
+//   inner index m = t_hi * 1024 + t_lo,  t_lo = 32 a + b,   output k = f_hi + RA * (c + 32 e)
+//   pass A  (thread <-> two t_lo 32 apart, all t_hi):
+//       y_{f_hi}[t_lo] = W_Nk^{t_lo f_hi} * sum_{t_hi} x[t_hi * 1024 + t_lo] W_RA^{t_hi f_hi}
+//   pass B1 (warp <-> (gate, f_hi), lane = b):  z[c][b] = W_1024^{b c} * sum_a y[32 a + b] W_32^{a c}
+//   pass B2 (same warp, lane = c):              X[f_hi + RA (c + 32 e)] = sum_b z[c][b] W_32^{b e}
+//
+// Arithmetic is packed: every float2 holds the SAME component (re or im) of TWO complex values
+// that go through identical butterflies (FADD2 / FMUL2 / FFMA2 on sm_100a: two lane-operations per
+// issue slot).  Pairs: pass A -- the thread's two t_lo (a even / a odd); B1 -- the even-a and odd-a
+// halves of a decimation-in-time radix-32; B2 -- the sum and difference halves of a
+// decimation-in-frequency radix-32, which are the even and odd output bins e.
+// Butterflies with a non-trivial constant twiddle use the 6-FMA form
+//   a +- W b = a +- wc * (b_r + t b_i,  b_i - t b_r),  t = tan,   (or the cotangent form when |ws| > |wc|)
+// with wc and t as FFMA2 immediates.
+//
+// Shared memory: 16 regions (one per B warp) of 16*65 8-byte slots + the B1->B2 twiddle table.
+//   A -> B1 :  slot (a'*2 + plane)*32 + b        holds (y[32(2a')+b], y[32(2a'+1)+b]).plane      (STS.64 / LDS.64)
+//   B1 -> B2:  slot  bb*65 + plane*32 + c        holds (z[c][bb], z[c][bb+16]).plane             (STS.32 / LDS.64)
+// Both are free of bank conflicts (the 65 pitch spreads the 4-byte transposed stores over all banks).
+//
+// S_dev layout written by this kernel: [r][q][f_hi][e][c]  (c = lane: every flush is 128 B per warp);
+// unpermute_kernel restores natural bin order at finalize.
+#pragma once
+#include "plspec_common.cuh"
+
+namespace plspec {
+
+constexpr int kRegionBytes = 16 * 65 * 8;                    // 8320
+constexpr int kFusedSmemBytes = 16 * kRegionBytes + 1024 * 8;  // + twB
+constexpr int kFusedThreads = 512;
+
+// ---- compile-time cos / sin of 2 pi k / 32 (float64, correctly rounded literals)
+constexpr double kCos32d[9] = {1.0,
+                               0.98078528040323044913,
+                               0.92387953251128675613,
+                               0.83146961230254523708,
+                               0.70710678118654752440,
+                               0.55557023301960222474,
+                               0.38268343236508977173,
+                               0.19509032201612826785,
+                               0.0};
+__host__ __device__ constexpr double cosd32(int k) {
+    k = ((k % 32) + 32) % 32;
+    if (k > 16) k = 32 - k;
+    return k > 8 ? -kCos32d[16 - k] : kCos32d[k];
+}
+__host__ __device__ constexpr double sind32(int k) { return cosd32(k - 8); }
+__host__ __device__ constexpr double absd(double x) { return x < 0 ? -x : x; }
+
+// ---- packed helpers: a float2 is two independent lanes
+__device__ __forceinline__ float2 padd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 psub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 pmul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 pfmak(float2 a, float k, float2 c) { return __ffma2_rn(a, make_float2(k, k), c); }
+__device__ __forceinline__ float2 pneg(float2 a) { return make_float2(-a.x, -a.y); }
+
+// (a, b) -> (a + W b, a - W b),  W = W_32^K32 = cos - i sin,  on two packed complex values at once
+template <int K32>
+__device__ __forceinline__ void bfly_dit(float2 &ar, float2 &ai, float2 &br, float2 &bi) {
+    if constexpr (K32 == 0) {
+        const float2 tr = br, ti = bi;
+        br = psub(ar, tr); bi = psub(ai, ti);
+        ar = padd(ar, tr); ai = padd(ai, ti);
+    } else if constexpr (K32 == 8) {                       // W = -i:  W b = (b_i, -b_r)
+        const float2 tr = bi, ti = br;
+        br = psub(ar, tr); bi = padd(ai, ti);
+        ar = padd(ar, tr); ai = psub(ai, ti);
+    } else {
+        constexpr double c = cosd32(K32), s = sind32(K32);
+        if constexpr (absd(c) >= absd(s)) {
+            constexpr float t = (float)(s / c), w = (float)c;   // W b = w (b_r + t b_i, b_i - t b_r)
+            const float2 p = pfmak(bi, t, br), q = pfmak(br, -t, bi);
+            br = pfmak(p, -w, ar); bi = pfmak(q, -w, ai);
+            ar = pfmak(p, w, ar);  ai = pfmak(q, w, ai);
+        } else {
+            constexpr float t = (float)(c / s), w = (float)s;   // W b = w (t b_r + b_i, t b_i - b_r)
+            const float2 p = pfmak(br, t, bi), q = pfmak(bi, t, pneg(br));
+            br = pfmak(p, -w, ar); bi = pfmak(q, -w, ai);
+            ar = pfmak(p, w, ar);  ai = pfmak(q, w, ai);
+        }
+    }
+}
+
+// Radix-2 decimation-in-time DFT of n = 1..16 packed points held at r[OFF..OFF+n), i[OFF..OFF+n) in
+// natural order; on return X[k] sits at index OFF + brev(k).
+template <int n, int OFF, int M>
+__device__ __forceinline__ void dft_packed(float2 (&r)[M], float2 (&i)[M]) {
+    constexpr int LOG = ilog2(n);
+    sfor<0, LOG>([&](auto s_) {
+        constexpr int half = 1 << decltype(s_)::value, len = 2 * half;
+        sfor<0, n / 2>([&](auto t_) {
+            constexpr int t = decltype(t_)::value;
+            constexpr int k = t % half, base = (t / half) * len;
+            constexpr int ia = OFF + brev<LOG>(base + k), ib = OFF + brev<LOG>(base + k + half);
+            bfly_dit<k * (32 / len)>(r[ia], i[ia], r[ib], i[ib]);
+        });
+    });
+}
+
+// last stage of a decimation-in-time radix-32: (.x, .y) = (E, O) -> (E + W O, E - W O), W = W_32^K32
+template <int K32>
+__device__ __forceinline__ void bfly_dit_halves(float2 &r, float2 &i) {
+    const float er = r.x, ei = i.x, orr = r.y, oi = i.y;
+    if constexpr (K32 == 0) {
+        r.x = er + orr; r.y = er - orr; i.x = ei + oi; i.y = ei - oi;
+    } else if constexpr (K32 == 8) {
+        r.x = er + oi; r.y = er - oi; i.x = ei - orr; i.y = ei + orr;
+    } else {
+        constexpr double c = cosd32(K32), s = sind32(K32);
+        float p, q, w;
+        if constexpr (absd(c) >= absd(s)) {
+            constexpr float t = (float)(s / c);
+            w = (float)c; p = fmaf(oi, t, orr); q = fmaf(orr, -t, oi);
+        } else {
+            constexpr float t = (float)(c / s);
+            w = (float)s; p = fmaf(orr, t, oi); q = fmaf(oi, t, -orr);
+        }
+        r.x = fmaf(p, w, er); r.y = fmaf(p, -w, er);
+        i.x = fmaf(q, w, ei); i.y = fmaf(q, -w, ei);
+    }
+}
+
+// first stage of a decimation-in-frequency radix-32: (.x, .y) = (z0, z1) -> (z0 + z1, (z0 - z1) W_32^K32)
+template <int K32>
+__device__ __forceinline__ void bfly_dif_halves(float2 &r, float2 &i) {
+    const float ur = r.x + r.y, ui = i.x + i.y, dr = r.x - r.y, di = i.x - i.y;
+    r.x = ur; i.x = ui;
+    if constexpr (K32 == 0) {
+        r.y = dr; i.y = di;
+    } else if constexpr (K32 == 8) {
+        r.y = di; i.y = -dr;
+    } else {
+        constexpr float c = (float)cosd32(K32), s = (float)sind32(K32);
+        r.y = fmaf(s, di, c * dr);
+        i.y = fmaf(-s, dr, c * di);
+    }
+}
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// ------------------------------------------------------------------------------------------
+template <int RA, int Q, int DT>
+__global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P) {
+    constexpr int NJ = 16 / RA;            // a' values per thread in pass A
+    constexpr int G = 16 / RA;             // gates per CTA
+    constexpr int LOGRA = ilog2(RA);
+    extern __shared__ __align__(16) unsigned char smem[];
+    const float2 *twB = reinterpret_cast<const float2 *>(smem + 16 * kRegionBytes);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = warp / RA, wa = warp % RA;       // pass A: warp `wa` of gate g;  pass B: (gate g, f_hi = wa)
+
+    // tile -> (gate group, q, IPP chunk)
+    int tile = blockIdx.x;
+    const int gg = tile % P.n_groups;
+    tile /= P.n_groups;
+    const int q = tile % Q;
+    const int chunk = tile / Q;
+    const int p_begin = (int)(((long long)chunk * P.n_ipp) / P.n_chunks);
+    const int p_end = (int)(((long long)(chunk + 1) * P.n_ipp) / P.n_chunks);
+    const int r = gg * G + g;
+    const bool gate_valid = r < P.R;
+    const int r_ld = gate_valid ? r : P.R - 1;     // ragged last group: recompute a valid gate, never flush it
+
+    {   // B1 -> B2 twiddles W_1024^{b c}, packed over (c', c'+16):  [(c'*2 + re/im)*32 + b]
+        float2 *dst = reinterpret_cast<float2 *>(smem + 16 * kRegionBytes);
+        for (int i = tid; i < 1024; i += kFusedThreads) dst[i] = __ldg(P.twB + i);
+    }
+    __syncthreads();
+
+    float2 acc[16];                        // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
+#pragma unroll
+    for (int j = 0; j < 16; j++) acc[j] = make_float2(0.f, 0.f);
+
+    unsigned char *const region = smem + warp * kRegionBytes;              // this warp's pass-B region
+    unsigned char *const gate_regions = smem + (g * RA) * kRegionBytes;    // regions of this gate (pass A target)
+    const long long gate_off = (long long)P.r0 + (long long)r_ld * P.stride;
+
+    for (int p = p_begin; p < p_end; p++) {
+        const float2 *Crow = P.C + (long long)p * P.L;
+        const long long voff = (long long)p * P.v_pitch + gate_off;
+        float2 xr[16], xi[16];
+        // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
+#pragma unroll
+        for (int jj = 0; jj < NJ; jj++) {
+            const int t_lo = 64 * (wa + RA * jj) + lane;
+#pragma unroll
+            for (int th = 0; th < RA; th++) {
+                const float2 d0 = load_decoded<Q, DT>(P, P.V, voff, Crow, th * 1024 + t_lo, q);
+                const float2 d1 = load_decoded<Q, DT>(P, P.V, voff, Crow, th * 1024 + t_lo + 32, q);
+                xr[jj * RA + th] = make_float2(d0.x, d1.x);
+                xi[jj * RA + th] = make_float2(d0.y, d1.y);
+            }
+        }
+        // DFT over t_hi, then y = X * W_Nk^{t_lo f_hi}
+        sfor<0, NJ>([&](auto jj_) {
+            constexpr int jj = decltype(jj_)::value;
+            dft_packed<RA, jj * RA>(xr, xi);
+        });
+        sfor<0, NJ>([&](auto jj_) {
+            constexpr int jj = decltype(jj_)::value;
+            const int ap = wa + RA * jj;
+            sfor<1, RA>([&](auto f_) {
+                constexpr int f = decltype(f_)::value;
+                constexpr int ph = jj * RA + brev<LOGRA>(f);
+                const float2 wr = __ldg(P.twA + ((ap * RA + f) * 2 + 0) * 32 + lane);
+                const float2 wi = __ldg(P.twA + ((ap * RA + f) * 2 + 1) * 32 + lane);
+                const float2 yr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
+                const float2 yi = pfma(xr[ph], wi, pmul(xi[ph], wr));
+                xr[ph] = yr; xi[ph] = yi;
+            });
+        });
+        // the gate's warps are done reading their regions for the previous window
+        if constexpr (RA == 1) __syncwarp(); else named_bar_sync(1 + g, RA * 32);
+        sfor<0, NJ>([&](auto jj_) {
+            constexpr int jj = decltype(jj_)::value;
+            const int ap = wa + RA * jj;
+            sfor<0, RA>([&](auto f_) {
+                constexpr int f = decltype(f_)::value;
+                constexpr int ph = jj * RA + brev<LOGRA>(f);
+                float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
+                dst[0] = xr[ph];
+                dst[32] = xi[ph];
+            });
+        });
+        if constexpr (RA == 1) __syncwarp(); else named_bar_sync(1 + g, RA * 32);
+
+        // ---- pass B1: lane = b; decimation-in-time radix-32 over a; .x = even a, .y = odd a
+        {
+            const float2 *src = reinterpret_cast<const float2 *>(region) + lane;
+#pragma unroll
+            for (int ap = 0; ap < 16; ap++) {
+                xr[ap] = src[(ap * 2) * 32];
+                xi[ap] = src[(ap * 2 + 1) * 32];
+            }
+        }
+        __syncwarp();
+        dft_packed<16, 0>(xr, xi);                               // (E[c'], O[c']) at brev4(c')
+        sfor<0, 16>([&](auto c_) {
+            constexpr int c = decltype(c_)::value;
+            constexpr int ph = brev<4>(c);
+            bfly_dit_halves<c>(xr[ph], xi[ph]);                  // (.x, .y) = (c', c' + 16)
+            const float2 wr = twB[(c * 2) * 32 + lane], wi = twB[(c * 2 + 1) * 32 + lane];
+            const float2 zr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
+            const float2 zi = pfma(xr[ph], wi, pmul(xi[ph], wr));
+            float *dst = reinterpret_cast<float *>(region + (lane & 15) * (65 * 8) + (lane >> 4) * 4);
+            dst[(c) * 2] = zr.x;
+            dst[(c + 16) * 2] = zr.y;
+            dst[(32 + c) * 2] = zi.x;
+            dst[(32 + c + 16) * 2] = zi.y;
+        });
+        __syncwarp();
+        // ---- pass B2: lane = c; decimation-in-frequency radix-32 over b; .x = b, .y = b + 16
+        {
+            const float2 *src = reinterpret_cast<const float2 *>(region) + lane;
+#pragma unroll
+            for (int bb = 0; bb < 16; bb++) {
+                xr[bb] = src[bb * 65];
+                xi[bb] = src[bb * 65 + 32];
+            }
+        }
+        sfor<0, 16>([&](auto b_) {
+            constexpr int bb = decltype(b_)::value;
+            bfly_dif_halves<bb>(xr[bb], xi[bb]);                 // (.x, .y) -> (even e, odd e) inputs
+        });
+        dft_packed<16, 0>(xr, xi);                               // (X[2 e'], X[2 e' + 1]) at brev4(e')
+#pragma unroll
+        for (int j = 0; j < 16; j++) {                           // |X|^2, accumulate (PAPER.md:79 Eq. 8, :115)
+            acc[j] = pfma(xr[j], xr[j], acc[j]);
+            acc[j] = pfma(xi[j], xi[j], acc[j]);
+        }
+    }
+
+    // ---- flush: S_dev[r][q][f_hi = wa][e][c = lane]
+    if (gate_valid) {
+        float *Srow = P.S + (((long long)r * Q + q) * RA + wa) * 1024 + lane;
+        sfor<0, 16>([&](auto j_) {
+            constexpr int j = decltype(j_)::value;
+            constexpr int e = 2 * brev<4>(j);
+            if (P.use_atomic) {
+                atomicAdd(Srow + e * 32, acc[j].x);
+                atomicAdd(Srow + (e + 1) * 32, acc[j].y);
+            } else {
+                Srow[e * 32] += acc[j].x;
+                Srow[(e + 1) * 32] += acc[j].y;
+            }
+        });
+    }
+}
+
+// S_out[r][q + Q (f_hi + RA (c + 32 e))] = S_dev[r][q][f_hi][e][c]   (fused layout), or
+// S_out[r][q + Q k]                      = S_dev[r][q][k]             (generic layout, RA = 0)
+__global__ void unpermute_kernel(const float *__restrict__ Sdev, float *__restrict__ Sout, int Q, int Nk, int RA,
+                                 long long total) {
+    const int N = Q * Nk;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
+         i += (long long)gridDim.x * blockDim.x) {
+        const long long r = i / N;
+        const int f = (int)(i - r * N);
+        const int q = f % Q, k = f / Q;
+        int src = k;
+        if (RA > 0) {
+            const int f_hi = k % RA, k_lo = k / RA;
+            src = (f_hi * 32 + (k_lo >> 5)) * 32 + (k_lo & 31);
+        }
+        Sout[i] = Sdev[(r * Q + q) * Nk + src];
+    }
+}
+
+}  // namespace plspec
