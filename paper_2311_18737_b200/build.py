@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libplspec.so")
 SOURCES = ["plspec_api.cu"]
-HEADERS = ["plspec_common.cuh", "plspec_kernels.cuh", os.path.join("..", "..", "include", "plspec.h")]
+HEADERS = ["plspec_common.cuh", "plspec_kernels.cuh", "plspec_fused.cuh", os.path.join("..", "..", "include", "plspec.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared",

@@ -36,7 +36,7 @@ struct plspec_ctx {
     int kind = 2;                    // 1 generic, 2 fused
     int Nk = 0, Q = 1, RA = 1;   // N = Q * Nk, Nk = 1024 * RA (fused)
     int gates_per_cta = 1, n_groups = 0;
-    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0;
+    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1;
     int block = 0;
     size_t smem = 0;
     int slots_per_wave = 0;          // n_sm * resident CTAs per SM
@@ -45,6 +45,9 @@ struct plspec_ctx {
     float  *S = nullptr;             // [R][Q][Nk]
     float  *S_tmp = nullptr;         // un-permute target when S_out is a host pointer
     float2 *twA = nullptr, *twB = nullptr, *twN = nullptr;
+    uint32_t *cbits = nullptr;       // packed code signs of the launch in flight (BPSK fast path)
+    long long cbits_words = 0;
+    int *not_bpsk = nullptr;         // device flag written by pack_codes_kernel
     // host pipeline
     cudaStream_t copy_stream = nullptr;
     Slot slot[kSlots];
@@ -156,6 +159,27 @@ int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long
     P.n_ipp = n_ipp;
     P.n_chunks = pick_chunks(h, n_ipp);
     P.use_atomic = P.n_chunks > 1 ? 1 : 0;
+    P.Cbits = nullptr; P.not_bpsk = nullptr;
+    if (h->kind == 2 && h->opt_bpsk && h->L == h->N) {
+        // code pre-pass: pack the signs of real +-1 codes (1 bit / sample instead of 8 bytes); the fused
+        // kernel falls back to the general complex decode when the flag says the codes are anything else
+        const long long words = (long long)n_ipp * h->Q * 512;
+        if (words > h->cbits_words) {
+            if (h->cbits) cudaFree(h->cbits);
+            h->cbits = nullptr; h->cbits_words = 0;
+            if (cudaMalloc((void **)&h->cbits, sizeof(uint32_t) * (size_t)words) != cudaSuccess) {
+                (void)cudaGetLastError();
+                return PLSPEC_ERR_ALLOC;
+            }
+            h->cbits_words = words;
+        }
+        PL_CUDA(h, cudaMemsetAsync(h->not_bpsk, 0, sizeof(int), stream));
+        pack_codes_kernel<<<(unsigned)((words + 255) / 256), 256, 0, stream>>>(dC, h->cbits, h->not_bpsk, h->L, h->Nk,
+                                                                              h->RA, h->Q, words);
+        PL_CUDA(h, cudaGetLastError());
+        h->stats.kernel_launches++;
+        P.Cbits = h->cbits; P.not_bpsk = h->not_bpsk;
+    }
     h->stats.ipp_chunks_last = P.n_chunks;
     const long long tiles = (long long)h->n_groups * h->Q * P.n_chunks;
     if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
@@ -290,6 +314,8 @@ void free_ctx(plspec_ctx *h) {
     if (h->twA) cudaFree(h->twA);
     if (h->twB) cudaFree(h->twB);
     if (h->twN) cudaFree(h->twN);
+    if (h->cbits) cudaFree(h->cbits);
+    if (h->not_bpsk) cudaFree(h->not_bpsk);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     if (h->work_done) cudaEventDestroy(h->work_done);
     (void)cudaGetLastError();
@@ -345,6 +371,7 @@ int plspec_create(int N, int code_len, int n_ranges, int r0, int stride, int ipp
         (void)cudaGetLastError();
         return fail(PLSPEC_ERR_CUDA);
     }
+    if (cudaMalloc((void **)&h->not_bpsk, sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_ALLOC); }
     if ((rc = build_tables(h)) != PLSPEC_OK) return fail(rc);
     if ((rc = select_kernel(h)) != PLSPEC_OK) return fail(rc);
     *out = h;
@@ -365,6 +392,7 @@ int plspec_configure(plspec_handle h, int option, int value) {
         }
         case PLSPEC_OPT_IPP_CHUNKS: h->opt_chunks = value; return PLSPEC_OK;
         case PLSPEC_OPT_H2D_BATCH:  h->opt_batch = value;  return PLSPEC_OK;
+        case PLSPEC_OPT_BPSK_PACK:  if (value > 1) return PLSPEC_ERR_INVALID_ARG; h->opt_bpsk = value; return PLSPEC_OK;
     }
     return PLSPEC_ERR_INVALID_ARG;
 }

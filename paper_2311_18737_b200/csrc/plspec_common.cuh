@@ -20,6 +20,8 @@ struct KParams {
     const float2 *twA;      // fused kernel, pass A -> B1: [a'][f_hi][re/im][lane] pairs W_Nk^{t_lo f_hi}
     const float2 *twB;      // fused kernel, pass B1 -> B2: [c'][re/im][lane] pairs W_1024^{b c}
     const float2 *twN;      // [N]: exp(-2 pi i e / N), full circle
+    const uint32_t *Cbits;  // fused kernel, BPSK fast path: [n_ipp][Q][512] packed code signs (or null)
+    const int    *not_bpsk; // device flag written by pack_codes_kernel: 0 = use Cbits
     long long     v_pitch;  // samples between successive IPP rows of V
     int N, Nk, Q, log2Nk;
     int L;                  // code_len

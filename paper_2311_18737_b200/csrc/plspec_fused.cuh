@@ -180,6 +180,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     }
     __syncthreads();
 
+    const bool bpsk = P.Cbits != nullptr && __ldg(P.not_bpsk) == 0;   // warp-uniform
     float2 acc[16];                        // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
 #pragma unroll
     for (int j = 0; j < 16; j++) acc[j] = make_float2(0.f, 0.f);
@@ -193,15 +194,33 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         const long long voff = (long long)p * P.v_pitch + gate_off;
         float2 xr[16], xi[16];
         // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
+        if (bpsk) {
+            sfor<0, NJ>([&](auto jj_) {
+                constexpr int jj = decltype(jj_)::value;
+                const int ap = wa + RA * jj;
+                const int t_lo = 64 * ap + lane;
+                uint32_t cw[Q];
 #pragma unroll
-        for (int jj = 0; jj < NJ; jj++) {
-            const int t_lo = 64 * (wa + RA * jj) + lane;
+                for (int j = 0; j < Q; j++) cw[j] = __ldg(P.Cbits + ((long long)p * Q + j) * 512 + ap * 32 + lane);
+                sfor<0, RA>([&](auto th_) {
+                    constexpr int th = decltype(th_)::value;
+                    const float2 d0 = load_decoded_bpsk<Q, DT, th * 2>(P, P.V, voff, cw, th * 1024 + t_lo, q);
+                    const float2 d1 = load_decoded_bpsk<Q, DT, th * 2 + 1>(P, P.V, voff, cw, th * 1024 + t_lo + 32, q);
+                    xr[jj * RA + th] = make_float2(d0.x, d1.x);
+                    xi[jj * RA + th] = make_float2(d0.y, d1.y);
+                });
+            });
+        } else {
 #pragma unroll
-            for (int th = 0; th < RA; th++) {
-                const float2 d0 = load_decoded<Q, DT>(P, P.V, voff, Crow, th * 1024 + t_lo, q);
-                const float2 d1 = load_decoded<Q, DT>(P, P.V, voff, Crow, th * 1024 + t_lo + 32, q);
-                xr[jj * RA + th] = make_float2(d0.x, d1.x);
-                xi[jj * RA + th] = make_float2(d0.y, d1.y);
+            for (int jj = 0; jj < NJ; jj++) {
+                const int t_lo = 64 * (wa + RA * jj) + lane;
+#pragma unroll
+                for (int th = 0; th < RA; th++) {
+                    const float2 d0 = load_decoded<Q, DT>(P, P.V, voff, Crow, th * 1024 + t_lo, q);
+                    const float2 d1 = load_decoded<Q, DT>(P, P.V, voff, Crow, th * 1024 + t_lo + 32, q);
+                    xr[jj * RA + th] = make_float2(d0.x, d1.x);
+                    xi[jj * RA + th] = make_float2(d0.y, d1.y);
+                }
             }
         }
         // DFT over t_hi, then y = X * W_Nk^{t_lo f_hi}

@@ -13,21 +13,9 @@ namespace plspec {
 
 // ------------------------------------------------------------------------------------------
 // decode + outer radix-Q butterfly for one inner index m (zero-pad reading A6)
-template <int Q, int DT>
-__device__ __forceinline__ float2 load_decoded(const KParams &P, const void *Vrow, long long voff,
-                                               const float2 *Crow, int m, int q) {
-    float2 d[Q];
-#pragma unroll
-    for (int j = 0; j < Q; j++) {
-        int t = m + j * P.Nk;
-        if (t < P.L) {
-            float2 z = load_voltage<DT>(Vrow, voff + t);
-            float2 c = __ldg(Crow + t);
-            d[j] = cmul_conj(z, c);
-        } else {
-            d[j] = make_float2(0.f, 0.f);
-        }
-    }
+// outer radix-Q decimation-in-frequency butterfly + twiddle W_N^{mq} on Q decoded samples d[j] = d(m + j Nk)
+template <int Q>
+__device__ __forceinline__ float2 outer_bfly(const KParams &P, const float2 (&d)[Q], int m, int q) {
     if constexpr (Q == 1) {
         return d[0];
     } else {
@@ -48,6 +36,63 @@ __device__ __forceinline__ float2 load_decoded(const KParams &P, const void *Vro
         if (q != 0) x = cmul(x, __ldg(P.twN + ((m * q) & (P.N - 1))));
         return x;
     }
+}
+
+template <int Q, int DT>
+__device__ __forceinline__ float2 load_decoded(const KParams &P, const void *Vrow, long long voff,
+                                               const float2 *Crow, int m, int q) {
+    float2 d[Q];
+#pragma unroll
+    for (int j = 0; j < Q; j++) {
+        int t = m + j * P.Nk;
+        if (t < P.L) {
+            float2 z = load_voltage<DT>(Vrow, voff + t);
+            float2 c = __ldg(Crow + t);
+            d[j] = cmul_conj(z, c);
+        } else {
+            d[j] = make_float2(0.f, 0.f);
+        }
+    }
+    return outer_bfly<Q>(P, d, m, q);
+}
+
+// BPSK fast path (code_len == N, every code sample exactly +-1 + 0j, found by pack_codes_kernel):
+// decode = sign flip.  cw[j] holds this thread's code bits of outer block j, bit `BIT` = 1 for -1.
+template <int Q, int DT, int BIT>
+__device__ __forceinline__ float2 load_decoded_bpsk(const KParams &P, const void *Vrow, long long voff,
+                                                    const uint32_t (&cw)[Q], int m, int q) {
+    float2 d[Q];
+#pragma unroll
+    for (int j = 0; j < Q; j++) {
+        float2 z = load_voltage<DT>(Vrow, voff + m + j * P.Nk);
+        const uint32_t s = (cw[j] << (31 - BIT)) & 0x80000000u;
+        d[j] = make_float2(__uint_as_float(__float_as_uint(z.x) ^ s), __uint_as_float(__float_as_uint(z.y) ^ s));
+    }
+    return outer_bfly<Q>(P, d, m, q);
+}
+
+// codes[n_ipp][L] (L == Q * 1024 * RA) -> bit-packed words in the fused kernel's pass-A thread order:
+// Cbits[p][j][ap * 32 + lane], bit (th * 2 + o) <-> t = j Nk + th 1024 + 64 ap + lane + 32 o.
+// *not_bpsk is set to 1 if any sample is not exactly +-1 + 0j (the fused kernel then decodes generally).
+__global__ void pack_codes_kernel(const float2 *__restrict__ C, uint32_t *__restrict__ Cbits, int *not_bpsk,
+                                  int L, int Nk, int RA, int Q, long long total_words) {
+    const long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= total_words) return;
+    const int lane = (int)(w & 31), ap = (int)((w >> 5) & 15);
+    const long long pj = w >> 9;
+    const int j = (int)(pj % Q);
+    const long long p = pj / Q;
+    const float2 *Crow = C + p * L + (long long)j * Nk + 64 * ap + lane;
+    uint32_t bits = 0;
+    bool ok = true;
+    for (int th = 0; th < RA; th++)
+        for (int o = 0; o < 2; o++) {
+            const float2 c = __ldg(Crow + th * 1024 + 32 * o);
+            ok = ok && (c.y == 0.f) && (c.x == 1.f || c.x == -1.f);
+            bits |= (c.x < 0.f ? 1u : 0u) << (th * 2 + o);
+        }
+    Cbits[w] = bits;
+    if (!ok) atomicOr(not_bpsk, 1);
 }
 
 __device__ __forceinline__ void tile_of_block(const KParams &P, int &r, int &q, int &p_begin, int &p_end) {

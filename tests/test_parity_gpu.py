@@ -30,10 +30,11 @@ def to_dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def run_gpu(w, V, C, *, kernel=pl.KERNEL_AUTO, chunks=0, splits=(None,), where="device", batch=0):
+def run_gpu(w, V, C, *, kernel=pl.KERNEL_AUTO, chunks=0, splits=(None,), where="device", batch=0, bpsk_pack=1):
     """One integration through the C ABI; returns S as float32 numpy [R][N]."""
     S = torch.full((w.n_ranges, w.N), -1.0, dtype=torch.float32, device="cuda")
-    with pl.Integrator.for_workload(w, kernel=kernel, ipp_chunks=chunks, h2d_batch=batch) as it:
+    with pl.Integrator.for_workload(w, kernel=kernel, ipp_chunks=chunks, h2d_batch=batch,
+                                     bpsk_pack=bpsk_pack) as it:
         bounds = [0] + [s for s in splits if s is not None] + [w.n_ipp]
         keep = []
         for a, b in zip(bounds[:-1], bounds[1:]):
@@ -113,7 +114,7 @@ def test_cfg5_scaled_stream_from_pinned_host():
     _, _, stats = check(w, V, C, where="pinned", batch=2)
     esz = 4
     assert stats["h2d_bytes"] == w.n_ipp * (w.span * esz + w.code_len * 8)   # span only, not whole IPPs
-    assert stats["kernel_launches"] == 5 + 1          # 5 staging batches + the un-permute at finalize
+    assert stats["kernel_launches"] == 5 * 2 + 1      # 5 staging batches x (code pre-pass + fused) + un-permute
 
 
 # ---- every FFT length, both kernels, awkward geometry --------------------------------------------
@@ -133,6 +134,31 @@ def test_all_lengths_fused(N, dtype):
     # and the two GPU implementations agree with each other
     S_gen, _ = run_gpu(w, V, C, kernel=pl.KERNEL_GENERIC)
     assert gate_metric(S_gen, S_ref).max() <= TOL
+
+
+@pytest.mark.parametrize("N", [1024, 4096, 16384, 65536])
+@pytest.mark.parametrize("dtype", [synth.CF32, synth.SC16])
+def test_bpsk_codes_packed_and_general_decode_agree(N, dtype):
+    """Binary phase codes (code_len == N) take the bit-packed sign-flip decode; the general complex
+    decode of the same inputs must give the same spectra, and one non-binary sample must switch the
+    whole launch to the general decode."""
+    R = 5 if N <= 4096 else 3
+    w, V, C = random_case(N, N, R, 2, 3, 3, dtype, complex_code=False)
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    S_fast, st = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED)
+    S_gen, st0 = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, bpsk_pack=0)
+    assert st["kernel_launches"] == st0["kernel_launches"] + 1          # the code pre-pass
+    assert gate_metric(S_fast, S_ref).max() <= TOL and gate_metric(S_gen, S_ref).max() <= TOL
+    C2 = C.copy()
+    C2[1, N // 3] = 1.0 + 0.5j                                          # not a binary phase code any more
+    S_ref2 = oracle.spectra(V, C2, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    S_mix, _ = run_gpu(w, V, C2, kernel=pl.KERNEL_FUSED)
+    assert gate_metric(S_mix, S_ref2).max() <= TOL
+    C3 = C.copy()
+    C3[0, 5] = 0.0                                                      # a zero chip is not +-1 either
+    S_ref3 = oracle.spectra(V, C3, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    S_z, _ = run_gpu(w, V, C3, kernel=pl.KERNEL_FUSED)
+    assert gate_metric(S_z, S_ref3).max() <= TOL
 
 
 def test_short_code_zero_padding():
