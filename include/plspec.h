@@ -49,10 +49,14 @@ enum { PLSPEC_OPT_KERNEL     = 1,   /* [0] 0 = auto, 1 = generic radix-2 kernel,
        PLSPEC_OPT_IPP_CHUNKS = 2,   /* [0] 0 = auto; else split each accumulate's IPPs over this many
                                        CTAs per gate (partial sums meet in S with fp32 atomics)     */
        PLSPEC_OPT_H2D_BATCH  = 3,   /* [0] 0 = auto; IPPs per host->device staging batch            */
-       PLSPEC_OPT_BPSK_PACK  = 4 }; /* [1] 1 = a pre-pass kernel bit-packs the codes of each accumulate when every
+       PLSPEC_OPT_BPSK_PACK  = 4,   /* [1] 1 = a pre-pass kernel bit-packs the codes of each accumulate when every
                                        sample is exactly +-1+0j (binary phase codes) and the fused kernel decodes
                                        by sign flip; any other code takes the general complex decode.
                                        0 = always decode generally.  Results are identical either way.   */
+       PLSPEC_OPT_STAGE      = 5 }; /* [1] 1 = the fused kernel prefetches each IPP's samples into shared memory
+                                       with bulk asynchronous copies whenever the run of samples one CTA needs
+                                       fits (N <= 16384 and, for complex64 input, N <= 8192); 0 = it always
+                                       loads voltages straight from global memory.  Results are identical.  */
 
 /* Counters since create (EXTENSION; used by bench.py for gpu_launches / h2d bytes). */
 typedef struct {

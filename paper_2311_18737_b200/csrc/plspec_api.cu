@@ -36,7 +36,8 @@ struct plspec_ctx {
     int kind = 2;                    // 1 generic, 2 fused
     int Nk = 0, Q = 1, RA = 1;   // N = Q * Nk, Nk = 1024 * RA (fused)
     int gates_per_cta = 1, n_groups = 0;
-    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1;
+    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1, opt_stage = 1;
+    bool staged = false;             // fused kernel reads voltages through the shared-memory stage
     int block = 0;
     size_t smem = 0;
     int slots_per_wave = 0;          // n_sm * resident CTAs per SM
@@ -76,24 +77,24 @@ namespace {
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
-template <int RA, int Q>
+template <int RA, int Q, bool ST>
 const void *fused_ptr(int dt) {
-    return dt == DT_CF32 ? (const void *)fused_kernel<RA, Q, DT_CF32>
-                         : (const void *)fused_kernel<RA, Q, DT_SC16>;
+    return dt == DT_CF32 ? (const void *)fused_kernel<RA, Q, DT_CF32, ST>
+                         : (const void *)fused_kernel<RA, Q, DT_SC16, ST>;
 }
 // the outer radix Q > 1 only occurs with the largest inner size (Nk = 16384, RA = 16)
-const void *fused_lookup(int RA, int Q, int dt) {
+const void *fused_lookup(int RA, int Q, int dt, bool st) {
     if (Q == 1) {
         switch (RA) {
-            case 1:  return fused_ptr<1, 1>(dt);
-            case 2:  return fused_ptr<2, 1>(dt);
-            case 4:  return fused_ptr<4, 1>(dt);
-            case 8:  return fused_ptr<8, 1>(dt);
-            case 16: return fused_ptr<16, 1>(dt);
+            case 1:  return st ? fused_ptr<1, 1, true>(dt) : fused_ptr<1, 1, false>(dt);
+            case 2:  return st ? fused_ptr<2, 1, true>(dt) : fused_ptr<2, 1, false>(dt);
+            case 4:  return st ? fused_ptr<4, 1, true>(dt) : fused_ptr<4, 1, false>(dt);
+            case 8:  return st ? fused_ptr<8, 1, true>(dt) : fused_ptr<8, 1, false>(dt);
+            case 16: return st ? fused_ptr<16, 1, true>(dt) : fused_ptr<16, 1, false>(dt);
         }
-    } else if (RA == 16) {
-        if (Q == 2) return fused_ptr<16, 2>(dt);
-        if (Q == 4) return fused_ptr<16, 4>(dt);
+    } else if (RA == 16 && !st) {
+        if (Q == 2) return fused_ptr<16, 2, false>(dt);
+        if (Q == 4) return fused_ptr<16, 4, false>(dt);
     }
     return nullptr;
 }
@@ -111,7 +112,12 @@ int select_kernel(plspec_ctx *h) {
         h->gates_per_cta = 16 / h->RA;
         h->block = kFusedThreads;
         h->smem = (size_t)kFusedSmemBytes;
-        h->kfunc = fused_lookup(h->RA, h->Q, dt);
+        // staged variant: the run of samples one CTA's gates touch per IPP must fit beside the exchange regions
+        const long long esz = dt == DT_SC16 ? 4 : 8;
+        const long long run = ((long long)(h->gates_per_cta - 1) * h->stride + h->L) * esz;
+        h->staged = h->opt_stage && h->Q == 1 && run + 32 <= (long long)kStageMaxBytes;
+        if (h->staged) h->smem = (size_t)kStageOff + (size_t)((run + 15) / 16 * 16 + 16);
+        h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged);
     } else {
         h->RA = 0;
         h->gates_per_cta = 1;
@@ -393,6 +399,14 @@ int plspec_configure(plspec_handle h, int option, int value) {
         case PLSPEC_OPT_IPP_CHUNKS: h->opt_chunks = value; return PLSPEC_OK;
         case PLSPEC_OPT_H2D_BATCH:  h->opt_batch = value;  return PLSPEC_OK;
         case PLSPEC_OPT_BPSK_PACK:  if (value > 1) return PLSPEC_ERR_INVALID_ARG; h->opt_bpsk = value; return PLSPEC_OK;
+        case PLSPEC_OPT_STAGE: {
+            if (value > 1) return PLSPEC_ERR_INVALID_ARG;
+            const int old = h->opt_stage;
+            h->opt_stage = value;
+            int rc = select_kernel(h);
+            if (rc != PLSPEC_OK) { h->opt_stage = old; (void)select_kernel(h); }
+            return rc;
+        }
     }
     return PLSPEC_ERR_INVALID_ARG;
 }

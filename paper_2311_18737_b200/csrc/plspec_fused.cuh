@@ -36,6 +36,10 @@ namespace plspec {
 
 constexpr int kRegionBytes = 16 * 65 * 8;                    // 8320
 constexpr int kFusedSmemBytes = 16 * kRegionBytes + 1024 * 8;  // + twB
+constexpr int kStageCtlBytes = 16;                             // mbarrier (8) + warp arrival counter (4)
+constexpr int kStageOff = kFusedSmemBytes + kStageCtlBytes;    // voltage stage of the ST variant (16-byte aligned)
+constexpr int kSmemMax = 227 * 1024;
+constexpr int kStageMaxBytes = kSmemMax - kStageOff;
 constexpr int kFusedThreads = 512;
 
 // ---- compile-time cos / sin of 2 pi k / 32 (float64, correctly rounded literals)
@@ -151,8 +155,15 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 }
 
 // ------------------------------------------------------------------------------------------
-template <int RA, int Q, int DT>
+// ST = true: the samples of IPP p that the CTA's gates touch (one contiguous run, overlapping windows
+// included once) are copied global -> shared by one cp.async.bulk per 32 KB while the CTA is still
+// transforming IPP p - 1; pass A then reads shared memory.  The copy starts at the 16-byte boundary at
+// or below the first sample and ends at the one at or above the last (CUDA allocations are 256-byte
+// granular, so the rounded run never leaves the allocation that holds the samples).
+template <int RA, int Q, int DT, bool ST>
 __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P) {
+    static_assert(!ST || Q == 1, "the staged variant holds one whole window run in shared memory");
+    constexpr int ESZ = DT == DT_CF32 ? 8 : 4;
     constexpr int NJ = 16 / RA;            // a' values per thread in pass A
     constexpr int G = 16 / RA;             // gates per CTA
     constexpr int LOGRA = ilog2(RA);
@@ -189,9 +200,45 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     unsigned char *const gate_regions = smem + (g * RA) * kRegionBytes;    // regions of this gate (pass A target)
     const long long gate_off = (long long)P.r0 + (long long)r_ld * P.stride;
 
+    // ---- ST: stage control.  mbar counts the bytes of one IPP's copy; cnt counts warps done reading it.
+    const uint32_t mbar = smem_u32(smem + kFusedSmemBytes);
+    int *const cnt = reinterpret_cast<int *>(smem + kFusedSmemBytes + 8);
+    const unsigned char *const stage = smem + kStageOff;
+    const long long run_off = (long long)P.r0 + (long long)(gg * G) * P.stride;   // first sample of the CTA's run
+    const int gates_here = (P.R - gg * G) < G ? (P.R - gg * G) : G;
+    const uint32_t run_bytes = (uint32_t)((gates_here - 1) * P.stride + P.L) * ESZ;
+    auto stage_issue = [&](int p) {                                        // one thread
+        const unsigned char *src = reinterpret_cast<const unsigned char *>(P.V) + ((long long)p * P.v_pitch + run_off) * ESZ;
+        const uint32_t mis = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15);
+        const uint32_t bytes = (mis + run_bytes + 15u) & ~15u;
+        mbar_arrive_expect_tx(mbar, bytes);
+        for (uint32_t off = 0; off < bytes; off += 32768u)
+            bulk_g2s(smem_u32(stage) + off, src - mis + off, (bytes - off) < 32768u ? (bytes - off) : 32768u, mbar);
+    };
+    if constexpr (ST) {
+        if (tid == 0) {
+            mbar_init(mbar, 1);
+            *cnt = 0;
+            fence_mbar_init();
+            fence_proxy_async();
+            if (p_begin < p_end) stage_issue(p_begin);
+        }
+        __syncthreads();
+    }
+    uint32_t parity = 0;
+    int arrivals_target = 15;                                              // 16 warps per IPP, 0-based last
+
     for (int p = p_begin; p < p_end; p++) {
         const float2 *Crow = P.C + (long long)p * P.L;
         const long long voff = (long long)p * P.v_pitch + gate_off;
+        VSrc vs;
+        vs.V = P.V; vs.voff = voff; vs.stage = stage; vs.sbase = 0;
+        if constexpr (ST) {
+            const uintptr_t a = reinterpret_cast<uintptr_t>(P.V) + (uintptr_t)(((long long)p * P.v_pitch + run_off) * ESZ);
+            vs.sbase = (int)((a & 15) / ESZ) + (r_ld - gg * G) * P.stride;
+            mbar_wait(mbar, parity);
+            parity ^= 1u;
+        }
         float2 xr[16], xi[16];
         // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
         if (bpsk) {
@@ -204,8 +251,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 for (int j = 0; j < Q; j++) cw[j] = __ldg(P.Cbits + ((long long)p * Q + j) * 512 + ap * 32 + lane);
                 sfor<0, RA>([&](auto th_) {
                     constexpr int th = decltype(th_)::value;
-                    const float2 d0 = load_decoded_bpsk<Q, DT, th * 2>(P, P.V, voff, cw, th * 1024 + t_lo, q);
-                    const float2 d1 = load_decoded_bpsk<Q, DT, th * 2 + 1>(P, P.V, voff, cw, th * 1024 + t_lo + 32, q);
+                    const float2 d0 = load_decoded_bpsk<Q, DT, th * 2, ST>(P, vs, cw, th * 1024 + t_lo, q);
+                    const float2 d1 = load_decoded_bpsk<Q, DT, th * 2 + 1, ST>(P, vs, cw, th * 1024 + t_lo + 32, q);
                     xr[jj * RA + th] = make_float2(d0.x, d1.x);
                     xi[jj * RA + th] = make_float2(d0.y, d1.y);
                 });
@@ -216,8 +263,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 const int t_lo = 64 * (wa + RA * jj) + lane;
 #pragma unroll
                 for (int th = 0; th < RA; th++) {
-                    const float2 d0 = load_decoded<Q, DT>(P, P.V, voff, Crow, th * 1024 + t_lo, q);
-                    const float2 d1 = load_decoded<Q, DT>(P, P.V, voff, Crow, th * 1024 + t_lo + 32, q);
+                    const float2 d0 = load_decoded<Q, DT, ST>(P, vs, Crow, th * 1024 + t_lo, q);
+                    const float2 d1 = load_decoded<Q, DT, ST>(P, vs, Crow, th * 1024 + t_lo + 32, q);
                     xr[jj * RA + th] = make_float2(d0.x, d1.x);
                     xi[jj * RA + th] = make_float2(d0.y, d1.y);
                 }
@@ -241,6 +288,20 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 xr[ph] = yr; xi[ph] = yi;
             });
         });
+        if constexpr (ST) {
+            // this warp has consumed its samples of IPP p; the last of the 16 warps starts the copy of IPP p + 1
+            __syncwarp();
+            if (lane == 0) {
+                __threadfence_block();
+                const int old = atomicAdd(cnt, 1);
+                if (old == arrivals_target && p + 1 < p_end) {
+                    __threadfence_block();
+                    fence_proxy_async();
+                    stage_issue(p + 1);
+                }
+            }
+            arrivals_target += 16;
+        }
         // the gate's warps are done reading their regions for the previous window
         if constexpr (RA == 1) __syncwarp(); else named_bar_sync(1 + g, RA * 32);
         sfor<0, NJ>([&](auto jj_) {

@@ -38,15 +38,33 @@ __device__ __forceinline__ float2 outer_bfly(const KParams &P, const float2 (&d)
     }
 }
 
-template <int Q, int DT>
-__device__ __forceinline__ float2 load_decoded(const KParams &P, const void *Vrow, long long voff,
-                                               const float2 *Crow, int m, int q) {
+// where one IPP's voltages come from: global memory (V + voff) or the CTA's shared-memory stage
+// (element index sbase + t; filled by cp.async.bulk in the fused kernel, plspec_fused.cuh)
+struct VSrc {
+    const void *V;
+    long long voff;
+    const unsigned char *stage;
+    int sbase;
+};
+
+template <int DT, bool STAGED>
+__device__ __forceinline__ float2 fetch_voltage(const VSrc &s, int t) {
+    if constexpr (STAGED) {
+        if constexpr (DT == DT_CF32) return reinterpret_cast<const float2 *>(s.stage)[s.sbase + t];
+        else return sc16_to_f32(reinterpret_cast<const uint32_t *>(s.stage)[s.sbase + t]);
+    } else {
+        return load_voltage<DT>(s.V, s.voff + t);
+    }
+}
+
+template <int Q, int DT, bool STAGED = false>
+__device__ __forceinline__ float2 load_decoded(const KParams &P, const VSrc &src, const float2 *Crow, int m, int q) {
     float2 d[Q];
 #pragma unroll
     for (int j = 0; j < Q; j++) {
         int t = m + j * P.Nk;
         if (t < P.L) {
-            float2 z = load_voltage<DT>(Vrow, voff + t);
+            float2 z = fetch_voltage<DT, STAGED>(src, t);
             float2 c = __ldg(Crow + t);
             d[j] = cmul_conj(z, c);
         } else {
@@ -58,13 +76,13 @@ __device__ __forceinline__ float2 load_decoded(const KParams &P, const void *Vro
 
 // BPSK fast path (code_len == N, every code sample exactly +-1 + 0j, found by pack_codes_kernel):
 // decode = sign flip.  cw[j] holds this thread's code bits of outer block j, bit `BIT` = 1 for -1.
-template <int Q, int DT, int BIT>
-__device__ __forceinline__ float2 load_decoded_bpsk(const KParams &P, const void *Vrow, long long voff,
-                                                    const uint32_t (&cw)[Q], int m, int q) {
+template <int Q, int DT, int BIT, bool STAGED = false>
+__device__ __forceinline__ float2 load_decoded_bpsk(const KParams &P, const VSrc &src, const uint32_t (&cw)[Q],
+                                                    int m, int q) {
     float2 d[Q];
 #pragma unroll
     for (int j = 0; j < Q; j++) {
-        float2 z = load_voltage<DT>(Vrow, voff + m + j * P.Nk);
+        float2 z = fetch_voltage<DT, STAGED>(src, m + j * P.Nk);
         const uint32_t s = (cw[j] << (31 - BIT)) & 0x80000000u;
         d[j] = make_float2(__uint_as_float(__float_as_uint(z.x) ^ s), __uint_as_float(__float_as_uint(z.y) ^ s));
     }
