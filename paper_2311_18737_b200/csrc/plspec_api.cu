@@ -111,7 +111,7 @@ int select_kernel(plspec_ctx *h) {
         h->RA = h->Nk / 1024;
         h->gates_per_cta = 16 / h->RA;
         h->block = kFusedThreads;
-        h->smem = (size_t)kFusedSmemBytes;
+        h->smem = (size_t)kStageOff;                       // exchange regions + control words
         // staged variant: the run of samples one CTA's gates touch per IPP must fit beside the exchange regions
         const long long esz = dt == DT_SC16 ? 4 : 8;
         const long long run = ((long long)(h->gates_per_cta - 1) * h->stride + h->L) * esz;

@@ -53,6 +53,18 @@ __device__ __forceinline__ float2 sc16_to_f32(uint32_t w) {
     return make_float2(re, im);
 }
 
+// two sc16 samples -> (re0, re1), (im0, im1), the subtraction done as one packed add each
+__device__ __forceinline__ void sc16_pair_to_f32(uint32_t w0, uint32_t w1, float2 &re, float2 &im) {
+    w0 ^= 0x80008000u;
+    w1 ^= 0x80008000u;
+    const float2 fr = make_float2(__uint_as_float(__byte_perm(w0, 0x4B000000u, 0x7610)),
+                                  __uint_as_float(__byte_perm(w1, 0x4B000000u, 0x7610)));
+    const float2 fi = make_float2(__uint_as_float(__byte_perm(w0, 0x4B000000u, 0x7632)),
+                                  __uint_as_float(__byte_perm(w1, 0x4B000000u, 0x7632)));
+    re = __fadd2_rn(fr, make_float2(-8421376.0f, -8421376.0f));
+    im = __fadd2_rn(fi, make_float2(-8421376.0f, -8421376.0f));
+}
+
 template <int DT>
 __device__ __forceinline__ float2 load_voltage(const void *V, long long idx) {
     if constexpr (DT == DT_CF32) {
@@ -93,6 +105,35 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(mbar)
                  : "memory");
+}
+
+// ---- tensor memory (TMEM) used as a per-thread constant store: 128 lanes x 512 columns x 32 bit per SM.
+// A warp reaches the 32 lanes of quadrant (warp % 4); `32x32b` gives thread i lane (quadrant base + i),
+// consecutive columns.  Address = (lane << 16) | column.
+__device__ __forceinline__ void tmem_alloc_512(uint32_t smem_result_addr) {          // one whole warp
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_result_addr) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_512(uint32_t taddr) {                     // one whole warp
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st4(uint32_t a, float x0, float x1, float x2, float x3) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "f"(x0), "f"(x1), "f"(x2), "f"(x3) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// 16 consecutive columns -> v[0..15]; the values may be used only after tmem_wait_ld16(v)
+__device__ __forceinline__ void tmem_ld16(uint32_t a, float (&v)[16]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]),
+                   "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
+                 : "r"(a));
+}
+__device__ __forceinline__ void tmem_wait_ld16(float (&v)[16]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]),
+                   "+f"(v[8]), "+f"(v[9]), "+f"(v[10]), "+f"(v[11]), "+f"(v[12]), "+f"(v[13]), "+f"(v[14]), "+f"(v[15]));
 }
 
 // compile-time loop

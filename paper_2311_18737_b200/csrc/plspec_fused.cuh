@@ -35,8 +35,8 @@
 namespace plspec {
 
 constexpr int kRegionBytes = 16 * 65 * 8;                    // 8320
-constexpr int kFusedSmemBytes = 16 * kRegionBytes + 1024 * 8;  // + twB
-constexpr int kStageCtlBytes = 16;                             // mbarrier (8) + warp arrival counter (4)
+constexpr int kFusedSmemBytes = 16 * kRegionBytes;
+constexpr int kStageCtlBytes = 16;                             // mbarrier (8) + warp arrival counter (4) + TMEM base (4)
 constexpr int kStageOff = kFusedSmemBytes + kStageCtlBytes;    // voltage stage of the ST variant (16-byte aligned)
 constexpr int kSmemMax = 227 * 1024;
 constexpr int kStageMaxBytes = kSmemMax - kStageOff;
@@ -168,8 +168,6 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     constexpr int G = 16 / RA;             // gates per CTA
     constexpr int LOGRA = ilog2(RA);
     extern __shared__ __align__(16) unsigned char smem[];
-    const float2 *twB = reinterpret_cast<const float2 *>(smem + 16 * kRegionBytes);
-
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = warp / RA, wa = warp % RA;       // pass A: warp `wa` of gate g;  pass B: (gate g, f_hi = wa)
 
@@ -185,11 +183,32 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     const bool gate_valid = r < P.R;
     const int r_ld = gate_valid ? r : P.R - 1;     // ragged last group: recompute a valid gate, never flush it
 
-    {   // B1 -> B2 twiddles W_1024^{b c}, packed over (c', c'+16):  [(c'*2 + re/im)*32 + b]
-        float2 *dst = reinterpret_cast<float2 *>(smem + 16 * kRegionBytes);
-        for (int i = tid; i < 1024; i += kFusedThreads) dst[i] = __ldg(P.twB + i);
-    }
+    // ---- twiddles live in tensor memory: every thread re-reads only constants it wrote itself
+    //   columns [4 e, 4 e + 4), e = jj (RA - 1) + f - 1:  pass A -> B1, W_Nk^{t_lo f} for the thread's two t_lo
+    //   columns [64 + 4 c', ..):                           B1 -> B2,   W_1024^{b c'}, W_1024^{b (c' + 16)}, b = lane
+    uint32_t *const tm_slot = reinterpret_cast<uint32_t *>(smem + kFusedSmemBytes + 12);
+    if (warp == 0) tmem_alloc_512(smem_u32(tm_slot));
+    tmem_fence_before_sync();
     __syncthreads();
+    tmem_fence_after_sync();
+    const uint32_t tm_base = *tm_slot;
+    const uint32_t tm = tm_base + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 128);
+    sfor<0, NJ>([&](auto jj_) {
+        constexpr int jj = decltype(jj_)::value;
+        const int ap = wa + RA * jj;
+        sfor<1, RA>([&](auto f_) {
+            constexpr int f = decltype(f_)::value;
+            const float2 wr = __ldg(P.twA + ((ap * RA + f) * 2 + 0) * 32 + lane);
+            const float2 wi = __ldg(P.twA + ((ap * RA + f) * 2 + 1) * 32 + lane);
+            tmem_st4(tm + 4 * (jj * (RA - 1) + f - 1), wr.x, wr.y, wi.x, wi.y);
+        });
+    });
+    sfor<0, 16>([&](auto c_) {
+        constexpr int c = decltype(c_)::value;
+        const float2 wr = __ldg(P.twB + (c * 2) * 32 + lane), wi = __ldg(P.twB + (c * 2 + 1) * 32 + lane);
+        tmem_st4(tm + 64 + 4 * c, wr.x, wr.y, wi.x, wi.y);
+    });
+    tmem_wait_st();
 
     const bool bpsk = P.Cbits != nullptr && __ldg(P.not_bpsk) == 0;   // warp-uniform
     float2 acc[16];                        // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
@@ -251,10 +270,15 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 for (int j = 0; j < Q; j++) cw[j] = __ldg(P.Cbits + ((long long)p * Q + j) * 512 + ap * 32 + lane);
                 sfor<0, RA>([&](auto th_) {
                     constexpr int th = decltype(th_)::value;
-                    const float2 d0 = load_decoded_bpsk<Q, DT, th * 2, ST>(P, vs, cw, th * 1024 + t_lo, q);
-                    const float2 d1 = load_decoded_bpsk<Q, DT, th * 2 + 1, ST>(P, vs, cw, th * 1024 + t_lo + 32, q);
-                    xr[jj * RA + th] = make_float2(d0.x, d1.x);
-                    xi[jj * RA + th] = make_float2(d0.y, d1.y);
+                    if constexpr (Q == 1) {
+                        load_pair_bpsk<DT, th * 2, th * 2 + 1, ST>(vs, cw[0], th * 1024 + t_lo, th * 1024 + t_lo + 32,
+                                                                    xr[jj * RA + th], xi[jj * RA + th]);
+                    } else {
+                        const float2 d0 = load_decoded_bpsk<Q, DT, th * 2, ST>(P, vs, cw, th * 1024 + t_lo, q);
+                        const float2 d1 = load_decoded_bpsk<Q, DT, th * 2 + 1, ST>(P, vs, cw, th * 1024 + t_lo + 32, q);
+                        xr[jj * RA + th] = make_float2(d0.x, d1.x);
+                        xi[jj * RA + th] = make_float2(d0.y, d1.y);
+                    }
                 });
             });
         } else {
@@ -275,19 +299,27 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             constexpr int jj = decltype(jj_)::value;
             dft_packed<RA, jj * RA>(xr, xi);
         });
-        sfor<0, NJ>([&](auto jj_) {
-            constexpr int jj = decltype(jj_)::value;
-            const int ap = wa + RA * jj;
-            sfor<1, RA>([&](auto f_) {
-                constexpr int f = decltype(f_)::value;
-                constexpr int ph = jj * RA + brev<LOGRA>(f);
-                const float2 wr = __ldg(P.twA + ((ap * RA + f) * 2 + 0) * 32 + lane);
-                const float2 wi = __ldg(P.twA + ((ap * RA + f) * 2 + 1) * 32 + lane);
-                const float2 yr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
-                const float2 yi = pfma(xr[ph], wi, pmul(xi[ph], wr));
-                xr[ph] = yr; xi[ph] = yi;
+        {
+            constexpr int NE = NJ * (RA - 1);                    // twiddle entries of this thread (0 when RA == 1)
+            sfor<0, (NE + 3) / 4>([&](auto g_) {
+                constexpr int gi = decltype(g_)::value;
+                float tw[16];
+                tmem_ld16(tm + 16 * gi, tw);
+                tmem_wait_ld16(tw);
+                sfor<0, 4>([&](auto k_) {
+                    constexpr int e = gi * 4 + decltype(k_)::value;
+                    if constexpr (e < NE) {
+                        constexpr int jj = e / (RA - 1), f = e % (RA - 1) + 1;
+                        constexpr int ph = jj * RA + brev<LOGRA>(f);
+                        constexpr int k = decltype(k_)::value;
+                        const float2 wr = make_float2(tw[4 * k], tw[4 * k + 1]), wi = make_float2(tw[4 * k + 2], tw[4 * k + 3]);
+                        const float2 yr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
+                        const float2 yi = pfma(xr[ph], wi, pmul(xi[ph], wr));
+                        xr[ph] = yr; xi[ph] = yi;
+                    }
+                });
             });
-        });
+        }
         if constexpr (ST) {
             // this warp has consumed its samples of IPP p; the last of the 16 warps starts the copy of IPP p + 1
             __syncwarp();
@@ -328,18 +360,25 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
         __syncwarp();
         dft_packed<16, 0>(xr, xi);                               // (E[c'], O[c']) at brev4(c')
-        sfor<0, 16>([&](auto c_) {
-            constexpr int c = decltype(c_)::value;
-            constexpr int ph = brev<4>(c);
-            bfly_dit_halves<c>(xr[ph], xi[ph]);                  // (.x, .y) = (c', c' + 16)
-            const float2 wr = twB[(c * 2) * 32 + lane], wi = twB[(c * 2 + 1) * 32 + lane];
-            const float2 zr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
-            const float2 zi = pfma(xr[ph], wi, pmul(xi[ph], wr));
-            float *dst = reinterpret_cast<float *>(region + (lane & 15) * (65 * 8) + (lane >> 4) * 4);
-            dst[(c) * 2] = zr.x;
-            dst[(c + 16) * 2] = zr.y;
-            dst[(32 + c) * 2] = zi.x;
-            dst[(32 + c + 16) * 2] = zi.y;
+        sfor<0, 4>([&](auto g_) {
+            constexpr int gi = decltype(g_)::value;
+            float tw[16];
+            tmem_ld16(tm + 64 + 16 * gi, tw);
+            tmem_wait_ld16(tw);
+            sfor<0, 4>([&](auto k_) {
+                constexpr int k = decltype(k_)::value;
+                constexpr int c = gi * 4 + k;
+                constexpr int ph = brev<4>(c);
+                bfly_dit_halves<c>(xr[ph], xi[ph]);              // (.x, .y) = (c', c' + 16)
+                const float2 wr = make_float2(tw[4 * k], tw[4 * k + 1]), wi = make_float2(tw[4 * k + 2], tw[4 * k + 3]);
+                const float2 zr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
+                const float2 zi = pfma(xr[ph], wi, pmul(xi[ph], wr));
+                float *dst = reinterpret_cast<float *>(region + (lane & 15) * (65 * 8) + (lane >> 4) * 4);
+                dst[(c) * 2] = zr.x;
+                dst[(c + 16) * 2] = zr.y;
+                dst[(32 + c) * 2] = zi.x;
+                dst[(32 + c + 16) * 2] = zi.y;
+            });
         });
         __syncwarp();
         // ---- pass B2: lane = c; decimation-in-frequency radix-32 over b; .x = b, .y = b + 16
@@ -378,6 +417,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             }
         });
     }
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc_512(tm_base);
 }
 
 // S_out[r][q + Q (f_hi + RA (c + 32 e))] = S_dev[r][q][f_hi][e][c]   (fused layout), or
