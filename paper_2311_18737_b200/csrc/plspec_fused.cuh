@@ -36,7 +36,8 @@ namespace plspec {
 
 constexpr int kRegionBytes = 16 * 65 * 8;                    // 8320
 constexpr int kFusedSmemBytes = 16 * kRegionBytes;
-constexpr int kStageCtlBytes = 16;                             // mbarrier (8) + warp arrival counter (4) + TMEM base (4)
+// control words: stage mbarrier (8) + warp arrival counter (4) + TMEM base (4) + 16 "regions free" mbarriers
+constexpr int kStageCtlBytes = 16 + 16 * 8;
 constexpr int kStageOff = kFusedSmemBytes + kStageCtlBytes;    // voltage stage of the ST variant (16-byte aligned)
 constexpr int kSmemMax = 227 * 1024;
 constexpr int kStageMaxBytes = kSmemMax - kStageOff;
@@ -234,17 +235,24 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         for (uint32_t off = 0; off < bytes; off += 32768u)
             bulk_g2s(smem_u32(stage) + off, src - mis + off, (bytes - off) < 32768u ? (bytes - off) : 32768u, mbar);
     };
-    if constexpr (ST) {
-        if (tid == 0) {
+    // free_mbar: the RA warps of gate g arrive once they have read their pass-B regions of a window (B2
+    // loads done); pass A of the next window waits on it before writing into those regions.
+    const uint32_t free_mbar = smem_u32(smem + kFusedSmemBytes + 16 + 8 * g);
+    if (tid == 0) {
+        for (int i = 0; i < G; i++) mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 8 * i), RA);
+        if constexpr (ST) {
             mbar_init(mbar, 1);
             *cnt = 0;
-            fence_mbar_init();
+        }
+        fence_mbar_init();
+        if constexpr (ST) {
             fence_proxy_async();
             if (p_begin < p_end) stage_issue(p_begin);
         }
-        __syncthreads();
     }
-    uint32_t parity = 0;
+    __syncthreads();
+    if (RA > 1 && lane == 0) mbar_arrive(free_mbar);                      // phase 0: the regions start out free
+    uint32_t parity = 0, free_parity = 0;
     int arrivals_target = 15;                                              // 16 warps per IPP, 0-based last
 
     for (int p = p_begin; p < p_end; p++) {
@@ -299,6 +307,36 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             constexpr int jj = decltype(jj_)::value;
             dft_packed<RA, jj * RA>(xr, xi);
         });
+        if constexpr (ST) {
+            // this warp has consumed its samples of IPP p; the last of the 16 warps starts the copy of IPP p + 1
+            __syncwarp();
+            if (lane == 0) {
+                __threadfence_block();
+                const int old = atomicAdd(cnt, 1);
+                if (old == arrivals_target && p + 1 < p_end) {
+                    __threadfence_block();
+                    fence_proxy_async();
+                    stage_issue(p + 1);
+                }
+            }
+            arrivals_target += 16;
+        }
+        // the gate's warps are done reading their regions for the previous window
+        if constexpr (RA == 1) {
+            __syncwarp();
+        } else {
+            mbar_wait(free_mbar, free_parity);
+            free_parity ^= 1u;
+        }
+        auto store_y = [&](auto jj_, auto f_) {                  // y_{f}[t_lo] -> region of pass-B warp (g, f)
+            constexpr int jj = decltype(jj_)::value, f = decltype(f_)::value;
+            constexpr int ph = jj * RA + brev<LOGRA>(f);
+            const int ap = wa + RA * jj;
+            float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
+            dst[0] = xr[ph];
+            dst[32] = xi[ph];
+        };
+        sfor<0, NJ>([&](auto jj_) { store_y(jj_, std::integral_constant<int, 0>{}); });
         {
             constexpr int NE = NJ * (RA - 1);                    // twiddle entries of this thread (0 when RA == 1)
             sfor<0, (NE + 3) / 4>([&](auto g_) {
@@ -316,37 +354,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                         const float2 yr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
                         const float2 yi = pfma(xr[ph], wi, pmul(xi[ph], wr));
                         xr[ph] = yr; xi[ph] = yi;
+                        store_y(std::integral_constant<int, jj>{}, std::integral_constant<int, f>{});
                     }
                 });
             });
         }
-        if constexpr (ST) {
-            // this warp has consumed its samples of IPP p; the last of the 16 warps starts the copy of IPP p + 1
-            __syncwarp();
-            if (lane == 0) {
-                __threadfence_block();
-                const int old = atomicAdd(cnt, 1);
-                if (old == arrivals_target && p + 1 < p_end) {
-                    __threadfence_block();
-                    fence_proxy_async();
-                    stage_issue(p + 1);
-                }
-            }
-            arrivals_target += 16;
-        }
-        // the gate's warps are done reading their regions for the previous window
-        if constexpr (RA == 1) __syncwarp(); else named_bar_sync(1 + g, RA * 32);
-        sfor<0, NJ>([&](auto jj_) {
-            constexpr int jj = decltype(jj_)::value;
-            const int ap = wa + RA * jj;
-            sfor<0, RA>([&](auto f_) {
-                constexpr int f = decltype(f_)::value;
-                constexpr int ph = jj * RA + brev<LOGRA>(f);
-                float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
-                dst[0] = xr[ph];
-                dst[32] = xi[ph];
-            });
-        });
         if constexpr (RA == 1) __syncwarp(); else named_bar_sync(1 + g, RA * 32);
 
         // ---- pass B1: lane = b; decimation-in-time radix-32 over a; .x = even a, .y = odd a
@@ -389,6 +401,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 xr[bb] = src[bb * 65];
                 xi[bb] = src[bb * 65 + 32];
             }
+        }
+        if constexpr (RA > 1) {                                  // this warp's region may be overwritten again
+            __syncwarp();
+            if (lane == 0) mbar_arrive(free_mbar);
         }
         sfor<0, 16>([&](auto b_) {
             constexpr int bb = decltype(b_)::value;
