@@ -155,6 +155,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 fused")
     ap.add_argument("--chunks", type=int, default=0)
+    ap.add_argument("--split", type=int, default=1, help="N > 16384: 1 decode pre-pass + scratch, 0 fully fused")
     ap.add_argument("--stage", type=int, default=1, help="1 shared-memory voltage stage where it fits, 0 direct loads")
     args = ap.parse_args()
     w = synth.CONFIGS[args.workload]
@@ -191,7 +192,7 @@ def main():
     S_dev = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
     S_pin = torch.empty((w.n_ranges, w.N), dtype=torch.float32).pin_memory()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
-    it = pl.Integrator.for_workload(w, kernel=args.kernel, ipp_chunks=args.chunks, stage=args.stage)
+    it = pl.Integrator.for_workload(w, kernel=args.kernel, ipp_chunks=args.chunks, stage=args.stage, split=args.split)
 
     def step_device(ev=None):
         if ev:

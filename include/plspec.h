@@ -53,10 +53,15 @@ enum { PLSPEC_OPT_KERNEL     = 1,   /* [0] 0 = auto, 1 = generic radix-2 kernel,
                                        sample is exactly +-1+0j (binary phase codes) and the fused kernel decodes
                                        by sign flip; any other code takes the general complex decode.
                                        0 = always decode generally.  Results are identical either way.   */
-       PLSPEC_OPT_STAGE      = 5 }; /* [1] 1 = the fused kernel prefetches each IPP's samples into shared memory
+       PLSPEC_OPT_STAGE      = 5, /* [1] 1 = the fused kernel prefetches each IPP's samples into shared memory
                                        with bulk asynchronous copies whenever the run of samples one CTA needs
                                        fits (N <= 16384 and, for complex64 input, N <= 8192); 0 = it always
                                        loads voltages straight from global memory.  Results are identical.  */
+       PLSPEC_OPT_SPLIT      = 6 }; /* [1] N > 16384 only.  1 = every window is decoded once by a pre-pass kernel (with
+                                       the outer radix-N/16384 butterfly) into a device scratch buffer (<= 4 GiB,
+                                       IPPs batched to fit) and the fused kernel transforms the N/16384 residues
+                                       as separate length-16384 windows; 0 = each (gate, residue) CTA decodes the
+                                       whole window itself (no scratch, N/16384 times the loads).               */
 
 /* Counters since create (EXTENSION; used by bench.py for gpu_launches / h2d bytes). */
 typedef struct {

@@ -36,7 +36,15 @@ struct plspec_ctx {
     int kind = 2;                    // 1 generic, 2 fused
     int Nk = 0, Q = 1, RA = 1;   // N = Q * Nk, Nk = 1024 * RA (fused)
     int gates_per_cta = 1, n_groups = 0;
-    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1, opt_stage = 1;
+    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1, opt_stage = 1, opt_split = 1;
+    // split path for N > 16384 (fused kernel only): decode + outer butterfly once into `xq`, then the
+    // Q == 1 fused kernel over R * Q virtual gates of length Nk
+    bool split = false;
+    const void *kfunc_split = nullptr;   // fused_kernel<16, 1, CF32, false>
+    float2 *xq = nullptr;                // [batch][R][Q][Nk]
+    long long xq_ipps = 0;               // IPPs the scratch holds
+    uint32_t *zero_bits = nullptr;       // identity "code" for step 2: all signs +
+    long long zero_bits_words = 0;
     bool staged = false;             // fused kernel reads voltages through the shared-memory stage
     int block = 0;
     size_t smem = 0;
@@ -118,8 +126,14 @@ int select_kernel(plspec_ctx *h) {
         h->staged = h->opt_stage && h->Q == 1 && run + 32 <= (long long)kStageMaxBytes;
         if (h->staged) h->smem = (size_t)kStageOff + (size_t)((run + 15) / 16 * 16 + 16);
         h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged);
+        h->split = h->opt_split && h->Q > 1;
+        if (h->split) {
+            h->kfunc_split = fused_lookup(16, 1, DT_CF32, false);
+            PL_CUDA(h, cudaFuncSetAttribute(h->kfunc_split, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageOff));
+        }
     } else {
         h->RA = 0;
+        h->split = false;
         h->gates_per_cta = 1;
         h->block = h->Nk / 2 < 32 ? 32 : (h->Nk / 2 > 512 ? 512 : h->Nk / 2);
         h->smem = (size_t)h->Nk * (sizeof(float2) + sizeof(float));
@@ -154,8 +168,12 @@ int pick_chunks(const plspec_ctx *h, int n_ipp) {
     return best;
 }
 
+int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp,
+                 cudaStream_t stream);
+
 int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0,
                       int n_ipp, cudaStream_t stream) {
+    if (h->kind == 2 && h->split) return launch_split(h, dV, dC, v_pitch, r0, n_ipp, stream);
     KParams P;
     P.V = dV; P.C = dC; P.S = h->S; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
     P.v_pitch = v_pitch;
@@ -192,6 +210,76 @@ int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long
     void *args[] = {&P};
     PL_CUDA(h, cudaLaunchKernel(h->kfunc, dim3((unsigned)tiles), dim3((unsigned)h->block), args, h->smem, stream));
     h->stats.kernel_launches++;
+    return PLSPEC_OK;
+}
+
+// N > 16384: predecode_kernel (every window decoded once, outer radix-Q butterfly) -> scratch -> fused
+// kernel with Q = 1 over R * Q virtual gates, in batches of IPPs that fit the scratch buffer.
+int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp,
+                 cudaStream_t stream) {
+    const long long per_ipp = (long long)h->R * h->N;                 // float2 elements of scratch per IPP
+    if (!h->xq) {
+        long long want = (4LL << 30) / (per_ipp * (long long)sizeof(float2));   // <= 4 GiB
+        if (want < 1) want = 1;
+        if (want > 64) want = 64;
+        if (h->opt_batch > 0 && want > h->opt_batch) want = h->opt_batch;
+        while (want >= 1 && cudaMalloc((void **)&h->xq, (size_t)(want * per_ipp) * sizeof(float2)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            h->xq = nullptr;
+            want /= 2;
+        }
+        if (!h->xq) return PLSPEC_ERR_ALLOC;
+        h->xq_ipps = want;
+        h->zero_bits_words = want * 512;
+        if (cudaMalloc((void **)&h->zero_bits, sizeof(uint32_t) * (size_t)h->zero_bits_words) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return PLSPEC_ERR_ALLOC;
+        }
+        PL_CUDA(h, cudaMemsetAsync(h->zero_bits, 0, sizeof(uint32_t) * (size_t)h->zero_bits_words, stream));
+        PL_CUDA(h, cudaMemsetAsync(h->not_bpsk, 0, sizeof(int), stream));
+    }
+    const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
+    for (int p0 = 0; p0 < n_ipp; p0 += (int)h->xq_ipps) {
+        const int nb = n_ipp - p0 < (int)h->xq_ipps ? n_ipp - p0 : (int)h->xq_ipps;
+        KParams P;
+        P.V = (const char *)dV + (size_t)p0 * (size_t)v_pitch * esz;
+        P.C = dC + (size_t)p0 * h->L;
+        P.S = h->S; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
+        P.Cbits = nullptr; P.not_bpsk = nullptr;
+        P.v_pitch = v_pitch;
+        P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
+        P.L = h->L; P.R = h->R; P.r0 = r0; P.stride = h->stride;
+        P.n_groups = h->R; P.n_ipp = nb; P.n_chunks = 1; P.use_atomic = 0;
+        const long long total = (long long)nb * h->R * h->Nk;
+        const unsigned blocks = (unsigned)((total + 255) / 256);
+        const bool sc = h->dtype == PLSPEC_SC16;
+        if (h->Q == 2) {
+            if (sc) predecode_kernel<2, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq, total);
+            else    predecode_kernel<2, DT_CF32><<<blocks, 256, 0, stream>>>(P, h->xq, total);
+        } else {
+            if (sc) predecode_kernel<4, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq, total);
+            else    predecode_kernel<4, DT_CF32><<<blocks, 256, 0, stream>>>(P, h->xq, total);
+        }
+        PL_CUDA(h, cudaGetLastError());
+        h->stats.kernel_launches++;
+        // step 2: R * Q virtual gates, window = Nk contiguous decoded samples, identity code
+        KParams F = P;
+        F.V = h->xq; F.C = dC;
+        F.Cbits = h->zero_bits; F.not_bpsk = h->not_bpsk;            // flag stays 0: sign-flip decode, no flips
+        F.v_pitch = per_ipp;
+        F.N = h->Nk; F.Q = 1; F.L = h->Nk;
+        F.R = h->R * h->Q; F.r0 = 0; F.stride = h->Nk;
+        F.n_groups = F.R;
+        F.n_chunks = pick_chunks(h, nb);
+        F.use_atomic = F.n_chunks > 1 ? 1 : 0;
+        h->stats.ipp_chunks_last = F.n_chunks;
+        const long long tiles = (long long)F.n_groups * F.n_chunks;
+        if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
+        void *args[] = {&F};
+        PL_CUDA(h, cudaLaunchKernel(h->kfunc_split, dim3((unsigned)tiles), dim3((unsigned)kFusedThreads), args,
+                                    (size_t)kStageOff, stream));
+        h->stats.kernel_launches++;
+    }
     return PLSPEC_OK;
 }
 
@@ -321,6 +409,8 @@ void free_ctx(plspec_ctx *h) {
     if (h->twB) cudaFree(h->twB);
     if (h->twN) cudaFree(h->twN);
     if (h->cbits) cudaFree(h->cbits);
+    if (h->xq) cudaFree(h->xq);
+    if (h->zero_bits) cudaFree(h->zero_bits);
     if (h->not_bpsk) cudaFree(h->not_bpsk);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     if (h->work_done) cudaEventDestroy(h->work_done);
@@ -399,6 +489,12 @@ int plspec_configure(plspec_handle h, int option, int value) {
         case PLSPEC_OPT_IPP_CHUNKS: h->opt_chunks = value; return PLSPEC_OK;
         case PLSPEC_OPT_H2D_BATCH:  h->opt_batch = value;  return PLSPEC_OK;
         case PLSPEC_OPT_BPSK_PACK:  if (value > 1) return PLSPEC_ERR_INVALID_ARG; h->opt_bpsk = value; return PLSPEC_OK;
+        case PLSPEC_OPT_SPLIT: {
+            if (value > 1) return PLSPEC_ERR_INVALID_ARG;
+            if (h->have_work) return PLSPEC_ERR_INVALID_ARG;
+            h->opt_split = value;
+            return select_kernel(h);
+        }
         case PLSPEC_OPT_STAGE: {
             if (value > 1) return PLSPEC_ERR_INVALID_ARG;
             const int old = h->opt_stage;

@@ -138,6 +138,42 @@ __global__ void pack_codes_kernel(const float2 *__restrict__ C, uint32_t *__rest
     if (!ok) atomicOr(not_bpsk, 1);
 }
 
+// ------------------------------------------------------------------------------------------
+// N > 16384 (outer radix Q = 2, 4), split path, step 1: decode every window ONCE and apply the outer
+// decimation-in-frequency butterfly for all Q residues at once,
+//     X[((p R + r) Q + q) Nk + m] = (sum_j d_{p,r}[m + j Nk] W_Q^{jq}) W_N^{mq},   d = V conj(C),
+// so that step 2 (the fused kernel on R Q "virtual gates" of length Nk, identity code) reads each decoded
+// sample once instead of every (gate, q) CTA decoding the whole window again.
+template <int Q, int DT>
+__global__ void __launch_bounds__(256) predecode_kernel(const KParams P, float2 *__restrict__ X, long long total) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // (p, r, m)
+    if (idx >= total) return;
+    const int m = (int)(idx % P.Nk);
+    const long long pr = idx / P.Nk;
+    const int r = (int)(pr % P.R);
+    const long long p = pr / P.R;
+    const float2 *Crow = P.C + p * P.L;
+    const long long voff = p * P.v_pitch + P.r0 + (long long)r * P.stride;
+    float2 d[Q];
+#pragma unroll
+    for (int j = 0; j < Q; j++) {
+        const int t = m + j * P.Nk;
+        d[j] = t < P.L ? cmul_conj(load_voltage<DT>(P.V, voff + t), __ldg(Crow + t)) : make_float2(0.f, 0.f);
+    }
+    float2 *out = X + (pr * Q) * P.Nk + m;
+    if constexpr (Q == 2) {
+        out[0] = cadd(d[0], d[1]);
+        out[P.Nk] = cmul(csub(d[0], d[1]), __ldg(P.twN + m));
+    } else {
+        static_assert(Q == 4, "outer radix must be 2 or 4");
+        const float2 e0 = cadd(d[0], d[2]), e1 = csub(d[0], d[2]), o0 = cadd(d[1], d[3]), o1 = csub(d[1], d[3]);
+        out[0] = cadd(e0, o0);
+        out[P.Nk] = cmul(make_float2(e1.x + o1.y, e1.y - o1.x), __ldg(P.twN + m));                 // e1 - i o1
+        out[2 * (long long)P.Nk] = cmul(csub(e0, o0), __ldg(P.twN + 2 * m));
+        out[3 * (long long)P.Nk] = cmul(make_float2(e1.x - o1.y, e1.y + o1.x), __ldg(P.twN + 3 * m)); // e1 + i o1
+    }
+}
+
 __device__ __forceinline__ void tile_of_block(const KParams &P, int &r, int &q, int &p_begin, int &p_end) {
     int tile = blockIdx.x;
     r = tile % P.R;
