@@ -156,7 +156,7 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 fused")
     ap.add_argument("--chunks", type=int, default=0)
     ap.add_argument("--split", type=int, default=1, help="N > 16384: 1 decode pre-pass + scratch, 0 fully fused")
-    ap.add_argument("--stage", type=int, default=1, help="1 shared-memory voltage stage where it fits, 0 direct loads")
+    ap.add_argument("--stage", type=int, default=1, help="1 shared-memory voltage stage where gates share samples, 2 wherever it fits, 0 direct loads")
     args = ap.parse_args()
     w = synth.CONFIGS[args.workload]
     if args.impl == "reference":

@@ -186,8 +186,8 @@ class Integrator:
                 plspec_configure(self.h, PLSPEC_OPT_H2D_BATCH, h2d_batch)
             if not bpsk_pack:
                 plspec_configure(self.h, PLSPEC_OPT_BPSK_PACK, 0)
-            if not stage:
-                plspec_configure(self.h, PLSPEC_OPT_STAGE, 0)
+            if stage != 1:
+                plspec_configure(self.h, PLSPEC_OPT_STAGE, stage)
             if not split:
                 plspec_configure(self.h, PLSPEC_OPT_SPLIT, 0)
         except Exception:

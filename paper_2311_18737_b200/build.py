@@ -36,7 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp,
+    cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("PLSPEC_NVCC_EXTRA", "").split(), *(["-Xptxas", "-v"] if verbose else []), "-o", tmp,
            *[os.path.join(CSRC, s) for s in SOURCES]]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)

@@ -123,7 +123,10 @@ int select_kernel(plspec_ctx *h) {
         // staged variant: the run of samples one CTA's gates touch per IPP must fit beside the exchange regions
         const long long esz = dt == DT_SC16 ? 4 : 8;
         const long long run = ((long long)(h->gates_per_cta - 1) * h->stride + h->L) * esz;
-        h->staged = h->opt_stage && h->Q == 1 && run + 32 <= (long long)kStageMaxBytes;
+        // opt_stage: 1 = where the run is shared by several gates of the CTA (measured: with one gate per CTA
+        // the stage only adds shared-memory traffic), 2 = wherever it fits, 0 = never
+        h->staged = h->opt_stage && h->Q == 1 && run + 32 <= (long long)kStageMaxBytes &&
+                    (h->gates_per_cta > 1 || h->opt_stage == 2);
         if (h->staged) h->smem = (size_t)kStageOff + (size_t)((run + 15) / 16 * 16 + 16);
         h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged);
         h->split = h->opt_split && h->Q > 1;
@@ -496,7 +499,7 @@ int plspec_configure(plspec_handle h, int option, int value) {
             return select_kernel(h);
         }
         case PLSPEC_OPT_STAGE: {
-            if (value > 1) return PLSPEC_ERR_INVALID_ARG;
+            if (value > 2) return PLSPEC_ERR_INVALID_ARG;
             const int old = h->opt_stage;
             h->opt_stage = value;
             int rc = select_kernel(h);

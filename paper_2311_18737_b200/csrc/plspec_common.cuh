@@ -53,16 +53,30 @@ __device__ __forceinline__ float2 sc16_to_f32(uint32_t w) {
     return make_float2(re, im);
 }
 
-// two sc16 samples -> (re0, re1), (im0, im1), the subtraction done as one packed add each
-__device__ __forceinline__ void sc16_pair_to_f32(uint32_t w0, uint32_t w1, float2 &re, float2 &im) {
-    w0 ^= 0x80008000u;
-    w1 ^= 0x80008000u;
+// all-ones if bit BIT of w is set, else 0: one shift shared by the four bits at BIT + 8k, then PRMT's
+// sign-replicate mode (selector nibble 8 + byte) smears the byte's top bit over the word
+template <int BIT>
+__device__ __forceinline__ uint32_t bit_mask(uint32_t w) {
+    constexpr uint32_t sel = 0x8888u + 0x1111u * (BIT >> 3);
+    uint32_t m;
+    asm("prmt.b32 %0, %1, 0, %2;" : "=r"(m) : "r"(w << (7 - (BIT & 7))), "n"(sel));   // __byte_perm drops selector bit 3
+    return m;
+}
+
+// two sc16 samples -> (re0, re1), (im0, im1), negated where the mask (0 or ~0) is set.  -x = ~x + 1 in
+// two's complement: complementing both halves of the word gives -x - 1, and the + 1 moves into the constant
+// of the packed subtraction (2^23 + 32768 or one less: adjacent fp32 bit patterns).
+__device__ __forceinline__ void sc16_pair_to_f32(uint32_t w0, uint32_t w1, uint32_t m0, uint32_t m1, float2 &re,
+                                                 float2 &im) {
+    w0 ^= 0x80008000u ^ m0;
+    w1 ^= 0x80008000u ^ m1;
     const float2 fr = make_float2(__uint_as_float(__byte_perm(w0, 0x4B000000u, 0x7610)),
                                   __uint_as_float(__byte_perm(w1, 0x4B000000u, 0x7610)));
     const float2 fi = make_float2(__uint_as_float(__byte_perm(w0, 0x4B000000u, 0x7632)),
                                   __uint_as_float(__byte_perm(w1, 0x4B000000u, 0x7632)));
-    re = __fadd2_rn(fr, make_float2(-8421376.0f, -8421376.0f));
-    im = __fadd2_rn(fi, make_float2(-8421376.0f, -8421376.0f));
+    const float2 k = make_float2(__uint_as_float(0xCB008000u + m0), __uint_as_float(0xCB008000u + m1));   // -(2^23 + 32768) [+ 1]
+    re = __fadd2_rn(fr, k);
+    im = __fadd2_rn(fi, k);
 }
 
 template <int DT>

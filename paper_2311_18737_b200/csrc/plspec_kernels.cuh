@@ -92,6 +92,7 @@ __device__ __forceinline__ float2 load_decoded_bpsk(const KParams &P, const VSrc
 // Q == 1 BPSK: the two samples t0, t1 of a packed pair at once -> xr = (re0, re1), xi = (im0, im1)
 template <int DT, int BIT0, int BIT1, bool STAGED>
 __device__ __forceinline__ void load_pair_bpsk(const VSrc &src, uint32_t cw, int t0, int t1, float2 &xr, float2 &xi) {
+    const uint32_t m0 = bit_mask<BIT0>(cw), m1 = bit_mask<BIT1>(cw);
     if constexpr (DT == DT_SC16) {
         uint32_t w0, w1;
         if constexpr (STAGED) {
@@ -101,17 +102,14 @@ __device__ __forceinline__ void load_pair_bpsk(const VSrc &src, uint32_t cw, int
             w0 = __ldg(reinterpret_cast<const uint32_t *>(src.V) + src.voff + t0);
             w1 = __ldg(reinterpret_cast<const uint32_t *>(src.V) + src.voff + t1);
         }
-        sc16_pair_to_f32(w0, w1, xr, xi);
+        sc16_pair_to_f32(w0, w1, m0, m1, xr, xi);
     } else {
         const float2 z0 = fetch_voltage<DT, STAGED>(src, t0), z1 = fetch_voltage<DT, STAGED>(src, t1);
-        xr = make_float2(z0.x, z1.x);
-        xi = make_float2(z0.y, z1.y);
+        xr = make_float2(__uint_as_float(__float_as_uint(z0.x) ^ (m0 & 0x80000000u)),
+                         __uint_as_float(__float_as_uint(z1.x) ^ (m1 & 0x80000000u)));
+        xi = make_float2(__uint_as_float(__float_as_uint(z0.y) ^ (m0 & 0x80000000u)),
+                         __uint_as_float(__float_as_uint(z1.y) ^ (m1 & 0x80000000u)));
     }
-    const uint32_t s0 = (cw << (31 - BIT0)) & 0x80000000u, s1 = (cw << (31 - BIT1)) & 0x80000000u;
-    xr.x = __uint_as_float(__float_as_uint(xr.x) ^ s0);
-    xi.x = __uint_as_float(__float_as_uint(xi.x) ^ s0);
-    xr.y = __uint_as_float(__float_as_uint(xr.y) ^ s1);
-    xi.y = __uint_as_float(__float_as_uint(xi.y) ^ s1);
 }
 
 // codes[n_ipp][L] (L == Q * 1024 * RA) -> bit-packed words in the fused kernel's pass-A thread order:

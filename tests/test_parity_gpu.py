@@ -173,11 +173,11 @@ def test_staged_and_direct_loads_agree(N, dtype, r0, stride):
     R = 2 * G + 1 if N <= 4096 else G + 1                 # ragged last gate group
     w, V, C = random_case(N, N, R, r0, stride, 3, dtype, pad=1, complex_code=(stride == 5))
     S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
-    S_st, _ = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, stage=1, chunks=2)
+    S_st, _ = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, stage=2, chunks=2)
     S_ld, _ = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, stage=0, chunks=2)
     assert gate_metric(S_st, S_ref).max() <= TOL
     assert np.allclose(S_st, S_ld, rtol=1e-5, atol=0)       # chunks meet through atomics: order may differ
-    S_st1, _ = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, stage=1, chunks=1)
+    S_st1, _ = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, stage=2, chunks=1)
     S_ld1, _ = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, stage=0, chunks=1)
     assert np.array_equal(S_st1, S_ld1)
 
