@@ -267,7 +267,7 @@ def main():
         flops_per_launch = w.fft_flops                              # 5 N log2 N x windows of one launch
         achieved = flops_per_launch / (kern_mean * 1e-3) / 1e12
         traffic = None
-        tfile = os.path.join(ROOT, "profiles", "traffic_bytes.json")
+        tfile = os.path.join(ROOT, "profiles", "traffic_bytes.txt")
         if os.path.exists(tfile):
             try:
                 traffic = json.load(open(tfile)).get(w.name)

@@ -253,15 +253,15 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
         P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
         P.L = h->L; P.R = h->R; P.r0 = r0; P.stride = h->stride;
         P.n_groups = h->R; P.n_ipp = nb; P.n_chunks = 1; P.use_atomic = 0;
-        const long long total = (long long)nb * h->R * h->Nk;
-        const unsigned blocks = (unsigned)((total + 255) / 256);
+        if (h->R > 65535 || nb > 65535) return PLSPEC_ERR_UNSUPPORTED;
+        const dim3 blocks((unsigned)(h->Nk / 512), (unsigned)h->R, (unsigned)nb);
         const bool sc = h->dtype == PLSPEC_SC16;
         if (h->Q == 2) {
-            if (sc) predecode_kernel<2, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq, total);
-            else    predecode_kernel<2, DT_CF32><<<blocks, 256, 0, stream>>>(P, h->xq, total);
+            if (sc) predecode_kernel<2, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq);
+            else    predecode_kernel<2, DT_CF32><<<blocks, 256, 0, stream>>>(P, h->xq);
         } else {
-            if (sc) predecode_kernel<4, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq, total);
-            else    predecode_kernel<4, DT_CF32><<<blocks, 256, 0, stream>>>(P, h->xq, total);
+            if (sc) predecode_kernel<4, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq);
+            else    predecode_kernel<4, DT_CF32><<<blocks, 256, 0, stream>>>(P, h->xq);
         }
         PL_CUDA(h, cudaGetLastError());
         h->stats.kernel_launches++;

@@ -142,34 +142,42 @@ __global__ void pack_codes_kernel(const float2 *__restrict__ C, uint32_t *__rest
 //     X[((p R + r) Q + q) Nk + m] = (sum_j d_{p,r}[m + j Nk] W_Q^{jq}) W_N^{mq},   d = V conj(C),
 // so that step 2 (the fused kernel on R Q "virtual gates" of length Nk, identity code) reads each decoded
 // sample once instead of every (gate, q) CTA decoding the whole window again.
+// grid = (Nk / 512, R, IPPs of the batch); a thread takes two adjacent m (one 16-byte store per residue)
 template <int Q, int DT>
-__global__ void __launch_bounds__(256) predecode_kernel(const KParams P, float2 *__restrict__ X, long long total) {
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // (p, r, m)
-    if (idx >= total) return;
-    const int m = (int)(idx % P.Nk);
-    const long long pr = idx / P.Nk;
-    const int r = (int)(pr % P.R);
-    const long long p = pr / P.R;
+__global__ void __launch_bounds__(256) predecode_kernel(const KParams P, float2 *__restrict__ X) {
+    const int m = 2 * (blockIdx.x * 256 + threadIdx.x);
+    const int r = blockIdx.y;
+    const long long p = blockIdx.z;
     const float2 *Crow = P.C + p * P.L;
     const long long voff = p * P.v_pitch + P.r0 + (long long)r * P.stride;
-    float2 d[Q];
+    float2 d[Q][2];
 #pragma unroll
-    for (int j = 0; j < Q; j++) {
-        const int t = m + j * P.Nk;
-        d[j] = t < P.L ? cmul_conj(load_voltage<DT>(P.V, voff + t), __ldg(Crow + t)) : make_float2(0.f, 0.f);
+    for (int j = 0; j < Q; j++)
+#pragma unroll
+        for (int k = 0; k < 2; k++) {
+            const int t = m + k + j * P.Nk;
+            d[j][k] = t < P.L ? cmul_conj(load_voltage<DT>(P.V, voff + t), __ldg(Crow + t)) : make_float2(0.f, 0.f);
+        }
+    float4 *out = reinterpret_cast<float4 *>(X + ((p * P.R + r) * Q) * P.Nk + m);
+    const long long qs = P.Nk / 2;                                   // float4 elements between residues
+    float2 x[Q][2];
+#pragma unroll
+    for (int k = 0; k < 2; k++) {
+        if constexpr (Q == 2) {
+            x[0][k] = cadd(d[0][k], d[1][k]);
+            x[1][k] = cmul(csub(d[0][k], d[1][k]), __ldg(P.twN + m + k));
+        } else {
+            static_assert(Q == 4, "outer radix must be 2 or 4");
+            const float2 e0 = cadd(d[0][k], d[2][k]), e1 = csub(d[0][k], d[2][k]);
+            const float2 o0 = cadd(d[1][k], d[3][k]), o1 = csub(d[1][k], d[3][k]);
+            x[0][k] = cadd(e0, o0);
+            x[1][k] = cmul(make_float2(e1.x + o1.y, e1.y - o1.x), __ldg(P.twN + (m + k)));        // e1 - i o1
+            x[2][k] = cmul(csub(e0, o0), __ldg(P.twN + 2 * (m + k)));
+            x[3][k] = cmul(make_float2(e1.x - o1.y, e1.y + o1.x), __ldg(P.twN + 3 * (m + k)));    // e1 + i o1
+        }
     }
-    float2 *out = X + (pr * Q) * P.Nk + m;
-    if constexpr (Q == 2) {
-        out[0] = cadd(d[0], d[1]);
-        out[P.Nk] = cmul(csub(d[0], d[1]), __ldg(P.twN + m));
-    } else {
-        static_assert(Q == 4, "outer radix must be 2 or 4");
-        const float2 e0 = cadd(d[0], d[2]), e1 = csub(d[0], d[2]), o0 = cadd(d[1], d[3]), o1 = csub(d[1], d[3]);
-        out[0] = cadd(e0, o0);
-        out[P.Nk] = cmul(make_float2(e1.x + o1.y, e1.y - o1.x), __ldg(P.twN + m));                 // e1 - i o1
-        out[2 * (long long)P.Nk] = cmul(csub(e0, o0), __ldg(P.twN + 2 * m));
-        out[3 * (long long)P.Nk] = cmul(make_float2(e1.x - o1.y, e1.y + o1.x), __ldg(P.twN + 3 * m)); // e1 + i o1
-    }
+#pragma unroll
+    for (int q = 0; q < Q; q++) out[q * qs] = make_float4(x[q][0].x, x[q][0].y, x[q][1].x, x[q][1].y);
 }
 
 __device__ __forceinline__ void tile_of_block(const KParams &P, int &r, int &q, int &p_begin, int &p_end) {
