@@ -121,6 +121,43 @@ def cpu_oracle_sample(w, V, C, target_s=12.0, steps=1):
                       f"({gates * w.n_ipp} windows, {dt:.1f} s per step, float64 radix-2, OpenMP over gates)"}, dt
 
 
+def cufft_pipeline(w, V_dev, C_dev, steps, flush):
+    """Comparison point, not the product (north_star): the unfused structure the paper describes
+     -- per IPP a decode multiply that writes `batch` to device memory, a batched cuFFT
+    (torch.fft -> cufftExecC2C) over its rows, and a power-accumulate pass -- on the same device-resident
+    inputs, timed with CUDA events like `value`."""
+    import torch
+    R, L, N = w.n_ranges, w.code_len, w.N
+    S = torch.zeros((R, N), dtype=torch.float32, device="cuda")
+
+    def step():
+        S.zero_()
+        for p in range(w.n_ipp):
+            if w.dtype == synth.SC16:
+                v = torch.view_as_complex(V_dev[p].to(torch.float32))          # sc16 -> fp32 (a1)
+            else:
+                v = V_dev[p]
+            win = v.as_strided((R, L), (w.stride, 1), w.r0)                     # overlapping windows (a2), a view
+            batch = win * C_dev[p].conj()                                       # K1 decode (a3)
+            X = torch.fft.fft(batch, n=N, dim=1)                                # K2 cuFFT, zero-padded to N (a4)
+            S.add_(torch.view_as_real(X).square().sum(dim=-1))                  # K3 power + accumulate (a5, a6)
+        return S
+
+    for _ in range(2):
+        step()
+    torch.cuda.synchronize()
+    ms = []
+    for _ in range(steps):
+        flush.fill_(4)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step()
+        e1.record()
+        e1.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    return float(np.mean(ms)), S
+
+
 def run_reference(args, w):
     """--impl reference: the oracle (the only 'reference implementation' this tier has)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -153,6 +190,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT + elementwise comparison pipeline")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 fused")
     ap.add_argument("--chunks", type=int, default=0)
     ap.add_argument("--split", type=int, default=1, help="N > 16384: 1 decode pre-pass + scratch, 0 fully fused")
@@ -250,6 +288,21 @@ def main():
         e2e_ms = float(np.sum(ts))
         barrier()
 
+    # ---- comparison point: unfused cuFFT pipeline (rank 0, N = 1 only)
+    cufft = None
+    if world == 1 and not args.no_cufft:
+        try:
+            cms, S_cu = cufft_pipeline(w, V_dev, C_dev, max(1, min(args.steps, 3)), flush)
+            step_device()
+            ref = S_cu.mean(dim=1, keepdim=True)
+            dev = float(((S_dev - S_cu).abs() / ref).max())
+            cufft = {"ms_per_step": cms, "value": w.windows / (cms * 1e-3), "unit": UNIT,
+                     "max_rel_dev_vs_fused": dev,
+                     "kind": "torch: decode multiply -> torch.fft.fft (cuFFT) -> power-accumulate, per IPP"}
+            del S_cu
+        except Exception as e:                                      # comparison only: never fails the bench
+            cufft = {"error": f"{type(e).__name__}: {e}"[:200]}
+
     # ---- max over ranks
     if dist is not None:
         t = torch.tensor([total_ms, e2e_ms or 0.0, float(np.mean(kern_ms))], device="cuda", dtype=torch.float64)
@@ -303,6 +356,8 @@ def main():
                            "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(w.n_ranges * w.N * 4),
                            "ms_per_step": e2e_ms / args.steps,
                            "realtime_factor": w.data_seconds * world * args.steps / (e2e_ms * 1e-3)}
+        if cufft is not None:
+            line["cufft_pipeline"] = cufft
         if world == 1 and not args.no_cpu_baseline:
             cb, _ = cpu_oracle_sample(w, V_np, C_np)
             line["cpu_baseline"] = cb
