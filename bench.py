@@ -193,6 +193,9 @@ def main():
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT + elementwise comparison pipeline")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 fused")
     ap.add_argument("--chunks", type=int, default=0)
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "ipp", "gates"],
+                    help="N > 1: independent integrations (weak scaling, no collective; default), or ONE "
+                         "integration sharded by IPP (sum all-reduce of S) / by range gate (all-gather)")
     ap.add_argument("--split", type=int, default=1, help="N > 16384: 1 decode pre-pass + scratch, 0 fully fused")
     ap.add_argument("--stage", type=int, default=1, help="1 shared-memory voltage stage where gates share samples, 2 wherever it fits, 0 direct loads")
     args = ap.parse_args()
@@ -222,27 +225,47 @@ def main():
 
     # ---- inputs: every rank integrates its own batch of the same shape (weak scaling, no
     # data-path collective: integrations are independent problems).
-    wr = synth.Workload(**{**w.__dict__, "seed": w.seed + 17 * rank})
+    from paper_2311_18737_b200 import shard
+    mode = args.shard if world > 1 else "replicas"
+    wr = synth.Workload(**{**w.__dict__, "seed": w.seed + (17 * rank if mode == "replicas" else 0)})
     V_np, C_np = synth.make_inputs(wr, full_ranges=w.n_ranges)
-    V_pin = torch.from_numpy(V_np).pin_memory()
-    C_pin = torch.from_numpy(C_np).pin_memory()
+    n_ipp_local, rows_local, r0_local = w.n_ipp, w.n_ranges, w.r0
+    if mode == "ipp":                                   # this rank's IPPs of the one integration
+        a, b = shard.split(w.n_ipp, rank, world)
+        V_np, C_np, n_ipp_local = V_np[a:b], C_np[a:b], b - a
+    elif mode == "gates":                               # this rank's gates; inputs replicated
+        gs = shard.gate_shard(w.n_ranges, w.r0, w.stride, w.code_len, rank, world)
+        rows_local, r0_local = gs.n_ranges, gs.r0
+    V_pin = torch.from_numpy(np.ascontiguousarray(V_np)).pin_memory()
+    C_pin = torch.from_numpy(np.ascontiguousarray(C_np)).pin_memory()
     V_dev, C_dev = V_pin.cuda(), C_pin.cuda()
-    S_dev = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
-    S_pin = torch.empty((w.n_ranges, w.N), dtype=torch.float32).pin_memory()
+    S_dev = torch.empty((rows_local, w.N), dtype=torch.float32, device="cuda")
+    S_pin = torch.empty((rows_local, w.N), dtype=torch.float32).pin_memory()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
-    it = pl.Integrator.for_workload(w, kernel=args.kernel, ipp_chunks=args.chunks, stage=args.stage, split=args.split)
+    it = pl.Integrator(w.N, w.code_len, rows_local, r0_local, w.stride, w.ipp_len, w.dtype, kernel=args.kernel,
+                       ipp_chunks=args.chunks, stage=args.stage, split=args.split)
+
+    def exchange(S):
+        if mode == "ipp":
+            return shard.sum_spectra(S)                 # the path's one exchange step (NCCL all-reduce)
+        if mode == "gates":
+            return shard.gather_gates(S, w.n_ranges)
+        return S
 
     def step_device(ev=None):
         if ev:
             ev[0].record()
-        it.accumulate(V_dev, C_dev, w.n_ipp)
+        it.accumulate(V_dev, C_dev, n_ipp_local)
         if ev:
             ev[1].record()
         it.finalize(S_dev)
+        exchange(S_dev)
 
     def step_host():
-        it.accumulate(V_pin, C_pin, w.n_ipp)
+        it.accumulate(V_pin, C_pin, n_ipp_local)
         it.finalize(S_pin)
+        if mode != "replicas":
+            exchange(S_pin.cuda())
 
     # ---- device-resident timing
     for _ in range(args.warmup):
@@ -304,16 +327,12 @@ def main():
             cufft = {"error": f"{type(e).__name__}: {e}"[:200]}
 
     # ---- max over ranks
-    if dist is not None:
-        t = torch.tensor([total_ms, e2e_ms or 0.0, float(np.mean(kern_ms))], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, e2e_max, kern_mean = [float(x) for x in t.cpu()]
-        e2e_ms = e2e_max if e2e_ms is not None else None
-    else:
-        kern_mean = float(np.mean(kern_ms))
+    total_ms, e2e_max, kern_mean = shard.max_over_ranks([total_ms, e2e_ms or 0.0, float(np.mean(kern_ms))],
+                                                        device="cuda")
+    e2e_ms = e2e_max if e2e_ms is not None else None
 
     if rank == 0:
-        windows_per_step = w.windows * world
+        windows_per_step = w.windows * (world if mode == "replicas" else 1)
         value = windows_per_step * args.steps / (total_ms * 1e-3)
         esz = 4 if w.dtype == synth.SC16 else 8
         h2d = w.n_ipp * (w.span * esz + w.code_len * 8)
@@ -329,17 +348,18 @@ def main():
         line = {
             "metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak",
+            "scaling": "weak" if mode == "replicas" else "strong",
             "vs_baseline": (value / PAPER_BEST_SPECTRA_PER_S) if w.name == "paper" else None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "N": w.N, "code_len": w.code_len, "n_ranges": w.n_ranges,
                        "stride": w.stride, "n_ipp": w.n_ipp, "ipp_len": w.ipp_len,
                        "input": "sc16" if w.dtype == synth.SC16 else "complex64",
                        "windows_per_step": w.windows, "l2": "flushed between steps (256 MB write)",
-                       "parallelism": f"{world} independent integrations (one per GPU)",
+                       "parallelism": (f"{world} independent integrations (one per GPU)" if mode == "replicas" else
+                                       f"one integration sharded by {mode} over {world} GPUs"),
                        "kernel": {1: "generic", 2: "fused"}[stats["kernel_kind"]],
                        "ipp_chunks": stats["ipp_chunks_last"]},
-            "realtime_factor": w.data_seconds * world * args.steps / (total_ms * 1e-3),
+            "realtime_factor": w.data_seconds * (world if mode == "replicas" else 1) * args.steps / (total_ms * 1e-3),
             "wall_s_timed_region": wall_s,
             "clocks": clocks,
             "gpu_launches": int(launches),
@@ -355,7 +375,8 @@ def main():
             line["e2e"] = {"value": windows_per_step * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
                            "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(w.n_ranges * w.N * 4),
                            "ms_per_step": e2e_ms / args.steps,
-                           "realtime_factor": w.data_seconds * world * args.steps / (e2e_ms * 1e-3)}
+                           "realtime_factor": w.data_seconds * (world if mode == "replicas" else 1) * args.steps
+                                              / (e2e_ms * 1e-3)}
         if cufft is not None:
             line["cufft_pipeline"] = cufft
         if world == 1 and not args.no_cpu_baseline:
