@@ -140,6 +140,16 @@ __device__ __forceinline__ void tmem_st4(uint32_t a, float x0, float x1, float x
     asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "f"(x0), "f"(x1), "f"(x2), "f"(x3) : "memory");
 }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// 8 consecutive columns -> v[0..7]; the values may be used only after tmem_wait_ld8(v)
+__device__ __forceinline__ void tmem_ld8(uint32_t a, float (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+                 : "r"(a));
+}
+__device__ __forceinline__ void tmem_wait_ld8(float (&v)[8]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]));
+}
 // 16 consecutive columns -> v[0..15]; the values may be used only after tmem_wait_ld16(v)
 __device__ __forceinline__ void tmem_ld16(uint32_t a, float (&v)[16]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"

@@ -302,7 +302,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 }
             }
         }
-        // DFT over t_hi, then y = X * W_Nk^{t_lo f_hi}
+        // DFT over t_hi, then y = X * W_Nk^{t_lo f_hi}; the first two twiddle pairs come in meanwhile
+        constexpr int NE = NJ * (RA - 1);                        // twiddle entries of this thread (0 when RA == 1)
+        float twe[8], two[8];                                    // even / odd groups of two entries
+        if constexpr (NE > 0) tmem_ld8(tm, twe);
         sfor<0, NJ>([&](auto jj_) {
             constexpr int jj = decltype(jj_)::value;
             dft_packed<RA, jj * RA>(xr, xi);
@@ -337,28 +340,26 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             dst[32] = xi[ph];
         };
         sfor<0, NJ>([&](auto jj_) { store_y(jj_, std::integral_constant<int, 0>{}); });
-        {
-            constexpr int NE = NJ * (RA - 1);                    // twiddle entries of this thread (0 when RA == 1)
-            sfor<0, (NE + 3) / 4>([&](auto g_) {
-                constexpr int gi = decltype(g_)::value;
-                float tw[16];
-                tmem_ld16(tm + 16 * gi, tw);
-                tmem_wait_ld16(tw);
-                sfor<0, 4>([&](auto k_) {
-                    constexpr int e = gi * 4 + decltype(k_)::value;
-                    if constexpr (e < NE) {
-                        constexpr int jj = e / (RA - 1), f = e % (RA - 1) + 1;
-                        constexpr int ph = jj * RA + brev<LOGRA>(f);
-                        constexpr int k = decltype(k_)::value;
-                        const float2 wr = make_float2(tw[4 * k], tw[4 * k + 1]), wi = make_float2(tw[4 * k + 2], tw[4 * k + 3]);
-                        const float2 yr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
-                        const float2 yi = pfma(xr[ph], wi, pmul(xi[ph], wr));
-                        xr[ph] = yr; xi[ph] = yi;
-                        store_y(std::integral_constant<int, jj>{}, std::integral_constant<int, f>{});
-                    }
-                });
+        sfor<0, (NE + 1) / 2>([&](auto g_) {
+            constexpr int gi = decltype(g_)::value;
+            float(&cur)[8] = (gi & 1) ? two : twe;
+            float(&nxt)[8] = (gi & 1) ? twe : two;
+            tmem_wait_ld8(cur);
+            if constexpr (gi + 1 < (NE + 1) / 2) tmem_ld8(tm + 8 * (gi + 1), nxt);
+            sfor<0, 2>([&](auto k_) {
+                constexpr int k = decltype(k_)::value;
+                constexpr int e = gi * 2 + k;
+                if constexpr (e < NE) {
+                    constexpr int jj = e / (RA - 1), f = e % (RA - 1) + 1;
+                    constexpr int ph = jj * RA + brev<LOGRA>(f);
+                    const float2 wr = make_float2(cur[4 * k], cur[4 * k + 1]), wi = make_float2(cur[4 * k + 2], cur[4 * k + 3]);
+                    const float2 yr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
+                    const float2 yi = pfma(xr[ph], wi, pmul(xi[ph], wr));
+                    xr[ph] = yr; xi[ph] = yi;
+                    store_y(std::integral_constant<int, jj>{}, std::integral_constant<int, f>{});
+                }
             });
-        }
+        });
         if constexpr (RA == 1) __syncwarp(); else named_bar_sync(1 + g, RA * 32);
 
         // ---- pass B1: lane = b; decimation-in-time radix-32 over a; .x = even a, .y = odd a
@@ -371,18 +372,20 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             }
         }
         __syncwarp();
+        tmem_ld8(tm + 64, twe);
         dft_packed<16, 0>(xr, xi);                               // (E[c'], O[c']) at brev4(c')
-        sfor<0, 4>([&](auto g_) {
+        sfor<0, 8>([&](auto g_) {
             constexpr int gi = decltype(g_)::value;
-            float tw[16];
-            tmem_ld16(tm + 64 + 16 * gi, tw);
-            tmem_wait_ld16(tw);
-            sfor<0, 4>([&](auto k_) {
+            float(&cur)[8] = (gi & 1) ? two : twe;
+            float(&nxt)[8] = (gi & 1) ? twe : two;
+            tmem_wait_ld8(cur);
+            if constexpr (gi + 1 < 8) tmem_ld8(tm + 64 + 8 * (gi + 1), nxt);
+            sfor<0, 2>([&](auto k_) {
                 constexpr int k = decltype(k_)::value;
-                constexpr int c = gi * 4 + k;
+                constexpr int c = gi * 2 + k;
                 constexpr int ph = brev<4>(c);
                 bfly_dit_halves<c>(xr[ph], xi[ph]);              // (.x, .y) = (c', c' + 16)
-                const float2 wr = make_float2(tw[4 * k], tw[4 * k + 1]), wi = make_float2(tw[4 * k + 2], tw[4 * k + 3]);
+                const float2 wr = make_float2(cur[4 * k], cur[4 * k + 1]), wi = make_float2(cur[4 * k + 2], cur[4 * k + 3]);
                 const float2 zr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
                 const float2 zi = pfma(xr[ph], wi, pmul(xi[ph], wr));
                 float *dst = reinterpret_cast<float *>(region + (lane & 15) * (65 * 8) + (lane >> 4) * 4);
