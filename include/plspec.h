@@ -117,6 +117,26 @@ int plspec_accumulate(plspec_handle h, const void *voltages, const void *codes,
  */
 int plspec_finalize(plspec_handle h, float *S_out);
 
+/*
+ * EXTENSION (the step after the hot path): per range gate of a finished spectrum,
+ * where the plasma lines are.  PAPER.md:40-45 (Eq. 1): the plasma line lies at +-f_r from the ion line, and
+ * f_r follows the electron density with range; PAPER.md:79 (Eq. 8): the estimate is the AVERAGE power.
+ *   S         [device] S[n_ranges][N] as written by plspec_finalize (sum over n_ipp pulses, natural bin order)
+ *   n_ipp     pulses summed in S (>= 1): reported powers are S / n_ipp
+ *   k_min     1 <= k_min < N/2: bins |f| < k_min (DC and the ion line) are left out
+ *   guard     >= 0: bins within `guard` of either line are left out of the noise floor
+ *   k_up      [device] int[n_ranges]: arg max of S over k_min <= f < N/2 (up-shifted line, +f_r)
+ *   k_dn      [device] int[n_ranges]: arg max over N/2 < f <= N - k_min (down-shifted line, bin N - f_r);
+ *             the lowest bin wins a tie in both
+ *   p_up,p_dn [device] float[n_ranges]: S / n_ipp at those bins
+ *   noise     [device] float[n_ranges]: mean of S / n_ipp over the other bins of [k_min, N - k_min] \ {N/2}
+ *   stream    cudaStream_t; one kernel is enqueued and the call returns without synchronising
+ * Caller owns every buffer.  Errors: PLSPEC_ERR_INVALID_ARG (null or host pointer, N not a power of two >= 16,
+ * range errors), PLSPEC_ERR_CUDA.  Needs no handle.
+ */
+int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, int guard,
+                   int *k_up, float *p_up, int *k_dn, float *p_dn, float *noise, void *stream);
+
 /* EXTENSIONS ------------------------------------------------------------------------------- */
 int plspec_reset(plspec_handle h);                        /* zero the accumulators, no output */
 int plspec_destroy(plspec_handle h);                      /* free everything; NULL is OK       */

@@ -37,7 +37,7 @@ LIB_PATH = os.path.join(_HERE, "libplspec.so")
 # every symbol include/plspec.h declares (tests check the library exports each one)
 EXPORTED_SYMBOLS = (
     "plspec_create", "plspec_accumulate", "plspec_finalize", "plspec_reset", "plspec_destroy",
-    "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_strerror",
+    "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_profile", "plspec_strerror",
     "plspec_version",
 )
 
@@ -86,7 +86,8 @@ def lib() -> ctypes.CDLL:
         L.plspec_strerror.argtypes = [ci]
         L.plspec_strerror.restype = ctypes.c_char_p
         L.plspec_version.restype = ctypes.c_char_p
-        for name in EXPORTED_SYMBOLS[:8]:
+        L.plspec_profile.argtypes = [vp, ci, ci, ci, ci, ci, vp, vp, vp, vp, vp, vp]
+        for name in EXPORTED_SYMBOLS[:9]:
             getattr(L, name).restype = ci
         _lib = L
     return _lib
@@ -145,6 +146,12 @@ def plspec_accumulate(h, voltages, codes, n_ipp, stream=None) -> None:
 
 def plspec_finalize(h, S_out) -> None:
     _check(h, lib().plspec_finalize(h, _ptr(S_out)), "plspec_finalize")
+
+
+def plspec_profile(S, n_ranges, N, n_ipp, k_min, guard, k_up, p_up, k_dn, p_dn, noise, stream=None) -> None:
+    _check(None, lib().plspec_profile(_ptr(S), int(n_ranges), int(N), int(n_ipp), int(k_min), int(guard), _ptr(k_up),
+                                      _ptr(p_up), _ptr(k_dn), _ptr(p_dn), _ptr(noise), _stream_ptr(stream)),
+           "plspec_profile")
 
 
 def plspec_reset(h) -> None:

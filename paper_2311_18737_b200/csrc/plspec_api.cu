@@ -560,6 +560,23 @@ int plspec_finalize(plspec_handle h, float *S_out) {
     return PLSPEC_OK;
 }
 
+int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, int guard, int *k_up, float *p_up,
+                   int *k_dn, float *p_dn, float *noise, void *stream) {
+    if (!S || !k_up || !p_up || !k_dn || !p_dn || !noise) return PLSPEC_ERR_INVALID_ARG;
+    if (!is_pow2(N) || N < 16 || n_ranges < 1 || n_ipp < 1 || k_min < 1 || k_min >= N / 2 || guard < 0)
+        return PLSPEC_ERR_INVALID_ARG;
+    const void *ptrs[] = {S, k_up, p_up, k_dn, p_dn, noise};
+    for (const void *p : ptrs) {                         // device (or managed) memory only
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { (void)cudaGetLastError(); return PLSPEC_ERR_CUDA; }
+        if (a.type != cudaMemoryTypeDevice && a.type != cudaMemoryTypeManaged) return PLSPEC_ERR_INVALID_ARG;
+    }
+    profile_kernel<<<(unsigned)n_ranges, 256, 0, (cudaStream_t)stream>>>(S, N, n_ipp, k_min, guard, k_up, p_up, k_dn,
+                                                                         p_dn, noise);
+    if (cudaGetLastError() != cudaSuccess) return PLSPEC_ERR_CUDA;
+    return PLSPEC_OK;
+}
+
 int plspec_reset(plspec_handle h) {
     if (!h) return PLSPEC_ERR_INVALID_ARG;
     cudaStream_t st = h->last_stream;

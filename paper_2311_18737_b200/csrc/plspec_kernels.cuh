@@ -180,6 +180,67 @@ __global__ void __launch_bounds__(256) predecode_kernel(const KParams P, float2 
     for (int q = 0; q < Q; q++) out[q * qs] = make_float4(x[q][0].x, x[q][0].y, x[q][1].x, x[q][1].y);
 }
 
+// ------------------------------------------------------------------------------------------
+// Post-integration products per range gate (SURVEY.md 8(f) NEXT-2; PAPER.md:40-45 Eq. 1, :79 Eq. 8):
+// arg max of S over the up-shifted half [k_min, N/2) and the down-shifted half (N/2, N - k_min] (lowest bin
+// wins a tie), the mean power S / n_ipp at those bins, and the mean of the remaining bins of
+// [k_min, N - k_min] \ {N/2} further than `guard` from either line (float64 sum).  One CTA per gate.
+struct ProfileBest { float v; int k; };
+__device__ __forceinline__ ProfileBest better(ProfileBest a, ProfileBest b) {
+    return (b.v > a.v || (b.v == a.v && b.k < a.k)) ? b : a;
+}
+__global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ S, int N, int n_ipp, int k_min, int guard,
+                                                      int *__restrict__ k_up, float *__restrict__ p_up,
+                                                      int *__restrict__ k_dn, float *__restrict__ p_dn,
+                                                      float *__restrict__ noise) {
+    __shared__ ProfileBest sb[2][8];
+    __shared__ double ssum[8];
+    __shared__ int scnt[8];
+    __shared__ int sk[2];
+    const float *row = S + (long long)blockIdx.x * N;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    ProfileBest up = {-1.f, 0x7fffffff}, dn = {-1.f, 0x7fffffff};      // S >= 0: any bin beats the start value
+    for (int f = k_min + tid; f <= N - k_min; f += 256) {
+        const ProfileBest c = {row[f], f};
+        if (f < N / 2) up = better(up, c);
+        else if (f > N / 2) dn = better(dn, c);
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        ProfileBest u = {__shfl_xor_sync(0xffffffffu, up.v, o), __shfl_xor_sync(0xffffffffu, up.k, o)};
+        ProfileBest d = {__shfl_xor_sync(0xffffffffu, dn.v, o), __shfl_xor_sync(0xffffffffu, dn.k, o)};
+        up = better(up, u); dn = better(dn, d);
+    }
+    if (lane == 0) { sb[0][warp] = up; sb[1][warp] = dn; }
+    __syncthreads();
+    if (tid == 0) {
+        for (int w = 1; w < 8; w++) { up = better(up, sb[0][w]); dn = better(dn, sb[1][w]); }
+        sk[0] = up.k; sk[1] = dn.k;
+        k_up[blockIdx.x] = up.k; k_dn[blockIdx.x] = dn.k;
+        p_up[blockIdx.x] = up.v / (float)n_ipp;
+        p_dn[blockIdx.x] = dn.v / (float)n_ipp;
+    }
+    __syncthreads();
+    const int ku = sk[0], kd = sk[1];
+    double acc = 0.0;
+    int cnt = 0;
+    for (int f = k_min + tid; f <= N - k_min; f += 256) {
+        const int du = f > ku ? f - ku : ku - f, dd = f > kd ? f - kd : kd - f;
+        if (f != N / 2 && du > guard && dd > guard) { acc += (double)row[f]; cnt++; }
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    }
+    if (lane == 0) { ssum[warp] = acc; scnt[warp] = cnt; }
+    __syncthreads();
+    if (tid == 0) {
+        for (int w = 1; w < 8; w++) { acc += ssum[w]; cnt += scnt[w]; }
+        noise[blockIdx.x] = cnt ? (float)(acc / (double)cnt / (double)n_ipp) : 0.f;
+    }
+}
+
 __device__ __forceinline__ void tile_of_block(const KParams &P, int &r, int &q, int &p_begin, int &p_end) {
     int tile = blockIdx.x;
     r = tile % P.R;

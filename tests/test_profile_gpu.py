@@ -1,0 +1,92 @@
+"""GPU parity of plspec_profile (post-integration products, NEXT-2) against oracle/profile_oracle.py on the
+same float32 spectra: line bins and powers bit-exact (integer decisions on values both sides hold exactly,
+one IEEE float32 division), noise floor to 1e-6 relative (float64 sums in a different order)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2311_18737_b200 import synth
+from paper_2311_18737_b200 import binding as pl
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+def run(S, n_ipp, k_min, guard, stream=None):
+    R, N = S.shape
+    Sd = torch.from_numpy(np.ascontiguousarray(S)).cuda()
+    ku = torch.full((R,), -7, dtype=torch.int32, device="cuda"); kd = torch.full_like(ku, -7)
+    pu = torch.full((R,), -1.0, dtype=torch.float32, device="cuda"); pd = torch.full_like(pu, -1.0)
+    nz = torch.full_like(pu, -1.0)
+    pl.plspec_profile(Sd, R, N, n_ipp, k_min, guard, ku, pu, kd, pd, nz, stream)
+    torch.cuda.synchronize()
+    return [t.cpu().numpy() for t in (ku, pu, kd, pd, nz)]
+
+
+def compare(S, n_ipp, k_min, guard):
+    got = run(S, n_ipp, k_min, guard)
+    ref = oracle.profile(S, n_ipp, k_min, guard)
+    for g, r, name in zip(got[:4], ref[:4], ("k_up", "p_up", "k_dn", "p_dn")):
+        assert np.array_equal(g, r), name
+    assert np.allclose(got[4], ref[4], rtol=1e-6, atol=0)
+    return got
+
+
+@pytest.mark.parametrize("N", [16, 64, 1024, 4096, 65536])
+def test_random_spectra_with_ties(N):
+    rng = np.random.default_rng(N)
+    R = 37 if N <= 4096 else 5
+    S = rng.integers(0, 50, size=(R, N)).astype(np.float32) * 0.25       # few distinct values: many ties
+    compare(S, 7, k_min=1, guard=0)
+    compare(S, 3, k_min=min(5, N // 2 - 1), guard=2)
+    S2 = rng.random((R, N)).astype(np.float32) * 1e6
+    compare(S2, 1000, k_min=min(3, N // 2 - 1), guard=1)
+
+
+def test_edges_of_both_halves_and_all_bins_guarded():
+    N = 32
+    S = np.ones((2, N), np.float32)
+    S[0, N // 2 - 1] = 9; S[0, N // 2 + 1] = 8; S[0, N // 2] = 100       # Nyquist ignored
+    S[1, 1] = 5; S[1, N - 1] = 6
+    got = compare(S, 1, k_min=1, guard=0)
+    assert got[0].tolist() == [15, 1] and got[2].tolist() == [17, 31]
+    got = compare(S, 1, k_min=1, guard=N)                                 # every bin within the guard
+    assert got[4].tolist() == [0.0, 0.0]
+
+
+def test_after_an_integration_recovers_the_chapman_profile():
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.CONFIGS["cfg2"], n_ranges=24, n_ipp=24), snr=0.5)
+    V, C = synth.make_inputs(w)
+    S = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+    with pl.Integrator.for_workload(w) as it:
+        it.accumulate(torch.from_numpy(V).cuda(), torch.from_numpy(C).cuda(), w.n_ipp)
+        it.finalize(S)
+    got = compare(S.cpu().numpy(), w.n_ipp, k_min=16, guard=3)            # oracle on the very same float32 S
+    want = synth.chapman_bins(synth.CONFIGS["cfg2"].n_ranges, w.N, np.arange(w.n_ranges))
+    assert np.abs(got[0] - np.rint(want)).max() <= 1
+    # and against the float64 path end to end: same bins from the oracle's own spectra
+    S64 = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride).astype(np.float32)
+    ref = oracle.profile(S64, w.n_ipp, 16, 3)
+    assert np.array_equal(got[0], ref[0]) and np.allclose(got[1], ref[1], rtol=1e-4)
+    assert np.allclose(got[4], ref[4], rtol=1e-4)
+
+
+def test_user_stream_and_argument_errors():
+    S = np.ones((3, 64), np.float32); S[:, 9] = 4; S[:, 50] = 3
+    st = torch.cuda.Stream()
+    got = run(S, 2, 2, 1, stream=st)
+    assert got[0].tolist() == [9, 9, 9] and got[3].tolist() == [1.5, 1.5, 1.5]
+    Sd = torch.ones((3, 64), dtype=torch.float32, device="cuda")
+    ki = torch.zeros(3, dtype=torch.int32, device="cuda"); pf = torch.zeros(3, dtype=torch.float32, device="cuda")
+    bad = [dict(N=48), dict(N=8), dict(n_ranges=0), dict(n_ipp=0), dict(k_min=0), dict(k_min=32), dict(guard=-1)]
+    base = dict(n_ranges=3, N=64, n_ipp=1, k_min=2, guard=0)
+    for b in bad:
+        a = {**base, **b}
+        with pytest.raises(pl.PlspecError) as e:
+            pl.plspec_profile(Sd, a["n_ranges"], a["N"], a["n_ipp"], a["k_min"], a["guard"], ki, pf, ki, pf, pf)
+        assert e.value.status == pl.PLSPEC_ERR_INVALID_ARG
+    with pytest.raises(pl.PlspecError):                                   # host pointer
+        pl.plspec_profile(np.ones((3, 64), np.float32), 3, 64, 1, 2, 0, ki, pf, ki, pf, pf)
+    with pytest.raises(pl.PlspecError):
+        pl.plspec_profile(Sd, 3, 64, 1, 2, 0, None, pf, ki, pf, pf)
