@@ -198,8 +198,12 @@ def main():
                          "integration sharded by IPP (sum all-reduce of S) / by range gate (all-gather)")
     ap.add_argument("--split", type=int, default=1, help="N > 16384: 1 decode pre-pass + scratch, 0 fully fused")
     ap.add_argument("--stage", type=int, default=1, help="1 shared-memory voltage stage where gates share samples, 2 wherever it fits, 0 direct loads")
+    ap.add_argument("--n-ipp", type=int, default=0, help="experiments: override the workload's IPP count")
+    ap.add_argument("--n-ranges", type=int, default=0, help="experiments: override the workload's gate count")
     args = ap.parse_args()
     w = synth.CONFIGS[args.workload]
+    if args.n_ipp or args.n_ranges:
+        w = synth.scaled(w, n_ranges=args.n_ranges or None, n_ipp=args.n_ipp or None, ipp_len=w.ipp_len)
     if args.impl == "reference":
         return run_reference(args, w)
     args.warmup = max(args.warmup, 3)

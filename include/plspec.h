@@ -46,8 +46,10 @@ enum { PLSPEC_OK = 0,
 
 /* plspec_configure options (EXTENSION; defaults in brackets). */
 enum { PLSPEC_OPT_KERNEL     = 1,   /* [0] 0 = auto, 1 = generic radix-2 kernel, 2 = fused kernel   */
-       PLSPEC_OPT_IPP_CHUNKS = 2,   /* [0] 0 = auto; else split each accumulate's IPPs over this many
-                                       CTAs per gate (partial sums meet in S with fp32 atomics)     */
+       PLSPEC_OPT_IPP_CHUNKS = 2,   /* [0] fused kernel: 0 = one CTA per SM, each an equal contiguous run of the
+                                       launch's (gate group, IPP) work items; else each gate group's IPPs are split
+                                       into this many equal runs, one CTA each.  Partial sums of a gate meet in S
+                                       through fp32 atomic adds either way.                               */
        PLSPEC_OPT_H2D_BATCH  = 3,   /* [0] 0 = auto; IPPs per host->device staging batch            */
        PLSPEC_OPT_BPSK_PACK  = 4,   /* [1] 1 = a pre-pass kernel bit-packs the codes of each accumulate when every
                                        sample is exactly +-1+0j (binary phase codes) and the fused kernel decodes
@@ -70,7 +72,7 @@ typedef struct {
     long long d2h_bytes;         /* bytes copied device->host by plspec_finalize            */
     long long ipps_accumulated;  /* IPPs accumulated since create                           */
     int       kernel_kind;       /* 1 = generic, 2 = fused (what `auto` resolved to)        */
-    int       ipp_chunks_last;   /* IPP chunks per gate used by the last accumulate         */
+    int       ipp_chunks_last;   /* IPP chunks per gate used by the last accumulate (0 = balanced runs) */
 } plspec_stats_t;
 
 /*

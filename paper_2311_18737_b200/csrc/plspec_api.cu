@@ -207,8 +207,20 @@ int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long
         h->stats.kernel_launches++;
         P.Cbits = h->cbits; P.not_bpsk = h->not_bpsk;
     }
+    long long tiles = (long long)h->n_groups * h->Q * P.n_chunks;
+    if (h->kind == 2) {
+        // fused kernel: flattened schedule.  auto = one CTA per resident slot, each an equal run of
+        // (tile, IPP) items; explicit chunks = that many equal IPP runs per tile, one CTA each
+        const long long items = (long long)h->n_groups * h->Q * n_ipp;
+        if (h->opt_chunks > 0) {
+            P.n_chunks = h->opt_chunks < n_ipp ? h->opt_chunks : n_ipp;
+            tiles = (long long)h->n_groups * h->Q * P.n_chunks;
+        } else {
+            P.n_chunks = 0;
+            tiles = items < h->slots_per_wave ? items : h->slots_per_wave;
+        }
+    }
     h->stats.ipp_chunks_last = P.n_chunks;
-    const long long tiles = (long long)h->n_groups * h->Q * P.n_chunks;
     if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
     void *args[] = {&P};
     PL_CUDA(h, cudaLaunchKernel(h->kfunc, dim3((unsigned)tiles), dim3((unsigned)h->block), args, h->smem, stream));
@@ -273,10 +285,17 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
         F.N = h->Nk; F.Q = 1; F.L = h->Nk;
         F.R = h->R * h->Q; F.r0 = 0; F.stride = h->Nk;
         F.n_groups = F.R;
-        F.n_chunks = pick_chunks(h, nb);
-        F.use_atomic = F.n_chunks > 1 ? 1 : 0;
+        const long long items = (long long)F.n_groups * nb;
+        long long tiles;
+        if (h->opt_chunks > 0) {
+            F.n_chunks = h->opt_chunks < nb ? h->opt_chunks : nb;
+            tiles = (long long)F.n_groups * F.n_chunks;
+        } else {
+            F.n_chunks = 0;
+            tiles = items < h->slots_per_wave ? items : h->slots_per_wave;
+        }
+        F.use_atomic = 1;
         h->stats.ipp_chunks_last = F.n_chunks;
-        const long long tiles = (long long)F.n_groups * F.n_chunks;
         if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
         void *args[] = {&F};
         PL_CUDA(h, cudaLaunchKernel(h->kfunc_split, dim3((unsigned)tiles), dim3((unsigned)kFusedThreads), args,

@@ -172,17 +172,17 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = warp / RA, wa = warp % RA;       // pass A: warp `wa` of gate g;  pass B: (gate g, f_hi = wa)
 
-    // tile -> (gate group, q, IPP chunk)
-    int tile = blockIdx.x;
-    const int gg = tile % P.n_groups;
-    tile /= P.n_groups;
-    const int q = tile % Q;
-    const int chunk = tile / Q;
-    const int p_begin = (int)(((long long)chunk * P.n_ipp) / P.n_chunks);
-    const int p_end = (int)(((long long)(chunk + 1) * P.n_ipp) / P.n_chunks);
-    const int r = gg * G + g;
-    const bool gate_valid = r < P.R;
-    const int r_ld = gate_valid ? r : P.R - 1;     // ragged last group: recompute a valid gate, never flush it
+    // ---- schedule: the launch's work items (tile, IPP), tile = (gate group, q), are numbered tile-major
+    // and CTA c takes the contiguous run [c T / n, (c + 1) T / n) of the T = tiles * n_ipp items: equal
+    // work for every CTA, accumulators flushed only where the run crosses into another tile.
+    const long long T = (long long)P.n_groups * Q * P.n_ipp;
+    const long long i0 = (long long)blockIdx.x * T / gridDim.x, i1 = ((long long)blockIdx.x + 1) * T / gridDim.x;
+    if (i0 >= i1) return;                          // uniform for the CTA; nothing allocated yet
+    const int tile0 = (int)(i0 / P.n_ipp);
+    const int p0 = (int)(i0 - (long long)tile0 * P.n_ipp);
+    // tile -> gate group and residue
+    auto group_of = [&](int t) { return Q == 1 ? t : t % P.n_groups; };
+    auto resid_of = [&](int t) { return Q == 1 ? 0 : t / P.n_groups; };
 
     // ---- twiddles live in tensor memory: every thread re-reads only constants it wrote itself
     //   columns [4 e, 4 e + 4), e = jj (RA - 1) + f - 1:  pass A -> B1, W_Nk^{t_lo f} for the thread's two t_lo
@@ -212,23 +212,20 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     tmem_wait_st();
 
     const bool bpsk = P.Cbits != nullptr && __ldg(P.not_bpsk) == 0;   // warp-uniform
-    float2 acc[16];                        // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
-#pragma unroll
-    for (int j = 0; j < 16; j++) acc[j] = make_float2(0.f, 0.f);
 
     unsigned char *const region = smem + warp * kRegionBytes;              // this warp's pass-B region
     unsigned char *const gate_regions = smem + (g * RA) * kRegionBytes;    // regions of this gate (pass A target)
-    const long long gate_off = (long long)P.r0 + (long long)r_ld * P.stride;
 
     // ---- ST: stage control.  mbar counts the bytes of one IPP's copy; cnt counts warps done reading it.
     const uint32_t mbar = smem_u32(smem + kFusedSmemBytes);
     int *const cnt = reinterpret_cast<int *>(smem + kFusedSmemBytes + 8);
     const unsigned char *const stage = smem + kStageOff;
-    const long long run_off = (long long)P.r0 + (long long)(gg * G) * P.stride;   // first sample of the CTA's run
-    const int gates_here = (P.R - gg * G) < G ? (P.R - gg * G) : G;
-    const uint32_t run_bytes = (uint32_t)((gates_here - 1) * P.stride + P.L) * ESZ;
-    auto stage_issue = [&](int p) {                                        // one thread
-        const unsigned char *src = reinterpret_cast<const unsigned char *>(P.V) + ((long long)p * P.v_pitch + run_off) * ESZ;
+    auto stage_issue = [&](int t, int pp) {                                // one thread: run of tile t, IPP pp
+        const int tg = group_of(t);
+        const int gates_here = (P.R - tg * G) < G ? (P.R - tg * G) : G;
+        const uint32_t run_bytes = (uint32_t)((gates_here - 1) * P.stride + P.L) * ESZ;
+        const long long roff = (long long)P.r0 + (long long)(tg * G) * P.stride;
+        const unsigned char *src = reinterpret_cast<const unsigned char *>(P.V) + ((long long)pp * P.v_pitch + roff) * ESZ;
         const uint32_t mis = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15);
         const uint32_t bytes = (mis + run_bytes + 15u) & ~15u;
         mbar_arrive_expect_tx(mbar, bytes);
@@ -247,7 +244,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         fence_mbar_init();
         if constexpr (ST) {
             fence_proxy_async();
-            if (p_begin < p_end) stage_issue(p_begin);
+            stage_issue(tile0, p0);
         }
     }
     __syncthreads();
@@ -255,7 +252,24 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     uint32_t parity = 0, free_parity = 0;
     int arrivals_target = 15;                                              // 16 warps per IPP, 0-based last
 
-    for (int p = p_begin; p < p_end; p++) {
+    int left = (int)(i1 - i0);                     // items still to do, this one included
+    int p_lo = p0;
+    for (int tile = tile0; left > 0; tile++, p_lo = 0) {                   // the tiles this CTA's run touches
+    const int p_hi = (P.n_ipp - p_lo) < left ? P.n_ipp : p_lo + left;
+    left -= p_hi - p_lo;
+    const bool more_tiles = left > 0;
+    const int gg = group_of(tile), q = resid_of(tile);
+    const int r = gg * G + g;
+    const int r_ld = r < P.R ? r : P.R - 1;        // ragged last group: recompute a valid gate, never flush it
+    const long long gate_off = (long long)P.r0 + (long long)r_ld * P.stride;
+    const long long run_off = (long long)P.r0 + (long long)(gg * G) * P.stride;   // first sample of the CTA's run
+    float2 acc[16];                                // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
+#pragma unroll
+    for (int j = 0; j < 16; j++) acc[j] = make_float2(0.f, 0.f);
+    for (int p = p_lo; p < p_hi; p++) {
+        const bool has_next = p + 1 < p_hi || more_tiles;
+        const int p_next = p + 1 < p_hi ? p + 1 : 0;
+        const int tile_next = p + 1 < p_hi ? tile : tile + 1;
         const float2 *Crow = P.C + (long long)p * P.L;
         const long long voff = (long long)p * P.v_pitch + gate_off;
         VSrc vs;
@@ -316,10 +330,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             if (lane == 0) {
                 __threadfence_block();
                 const int old = atomicAdd(cnt, 1);
-                if (old == arrivals_target && p + 1 < p_end) {
+                if (old == arrivals_target && has_next) {
                     __threadfence_block();
                     fence_proxy_async();
-                    stage_issue(p + 1);
+                    stage_issue(tile_next, p_next);
                 }
             }
             arrivals_target += 16;
@@ -420,22 +434,18 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             acc[j] = pfma(xi[j], xi[j], acc[j]);
         }
     }
-
-    // ---- flush: S_dev[r][q][f_hi = wa][e][c = lane]
-    if (gate_valid) {
+    // ---- flush: S_dev[r][q][f_hi = wa][e][c = lane]; other CTAs may hold the rest of this tile's IPPs
+    if (r < P.R) {
         float *Srow = P.S + (((long long)r * Q + q) * RA + wa) * 1024 + lane;
         sfor<0, 16>([&](auto j_) {
             constexpr int j = decltype(j_)::value;
             constexpr int e = 2 * brev<4>(j);
-            if (P.use_atomic) {
-                atomicAdd(Srow + e * 32, acc[j].x);
-                atomicAdd(Srow + (e + 1) * 32, acc[j].y);
-            } else {
-                Srow[e * 32] += acc[j].x;
-                Srow[(e + 1) * 32] += acc[j].y;
-            }
+            atomicAdd(Srow + e * 32, acc[j].x);
+            atomicAdd(Srow + (e + 1) * 32, acc[j].y);
         });
     }
+    }
+
     tmem_fence_before_sync();
     __syncthreads();
     if (warp == 0) tmem_dealloc_512(tm_base);
