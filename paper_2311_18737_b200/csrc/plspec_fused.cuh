@@ -112,6 +112,53 @@ __device__ __forceinline__ void dft_packed(float2 (&r)[M], float2 (&i)[M]) {
     });
 }
 
+// Last stage of the packed 16-point DIT fused with |X|^2 (Eq. 8): the butterfly outputs a +- W b
+// are never formed.  |a +- W b|^2 = (|a|^2 + |b|^2) +- 2 Re(conj(a) W b), so per butterfly two running sums
+//   accS += |a|^2 + |b|^2,   accC += a_r p + a_i q   with  W b = w (p, q)  (tangent / cotangent form)
+// replace four adds and four multiply-adds by six multiply-adds (eight with a non-trivial twiddle instead of
+// ten); the two spectra values are accS +- 2 w accC at flush time (kPow2w).
+template <int K32>
+__device__ __forceinline__ void bfly_power(float2 ar, float2 ai, float2 br, float2 bi, float2 &accS, float2 &accC) {
+    accS = pfma(ar, ar, accS); accS = pfma(ai, ai, accS);
+    accS = pfma(br, br, accS); accS = pfma(bi, bi, accS);
+    if constexpr (K32 == 0) {
+        accC = pfma(ar, br, accC); accC = pfma(ai, bi, accC);
+    } else if constexpr (K32 == 8) {                       // W b = (b_i, -b_r)
+        accC = pfma(ar, bi, accC); accC = pfma(ai, pneg(br), accC);
+    } else {
+        constexpr double c = cosd32(K32), sn = sind32(K32);
+        if constexpr (absd(c) >= absd(sn)) {
+            constexpr float t = (float)(sn / c);
+            const float2 p = pfmak(bi, t, br), q = pfmak(br, -t, bi);
+            accC = pfma(ar, p, accC); accC = pfma(ai, q, accC);
+        } else {
+            constexpr float t = (float)(c / sn);
+            const float2 p = pfmak(br, t, bi), q = pfmak(bi, t, pneg(br));
+            accC = pfma(ar, p, accC); accC = pfma(ai, q, accC);
+        }
+    }
+}
+// 2 w of the butterfly above: w = 1 for the trivial twiddles, else cos or sin (whichever is larger in modulus)
+__host__ __device__ constexpr float pow2w(int K32) {
+    if (K32 == 0 || K32 == 8) return 2.0f;
+    const double c = cosd32(K32), sn = sind32(K32);
+    return (float)(2.0 * (absd(c) >= absd(sn) ? c : sn));
+}
+
+// the first LOG - 1 stages of dft_packed<16, 0>
+template <int M>
+__device__ __forceinline__ void dft_packed16_head(float2 (&r)[M], float2 (&i)[M]) {
+    sfor<0, 3>([&](auto s_) {
+        constexpr int half = 1 << decltype(s_)::value, len = 2 * half;
+        sfor<0, 8>([&](auto t_) {
+            constexpr int t = decltype(t_)::value;
+            constexpr int k = t % half, base = (t / half) * len;
+            constexpr int ia = brev<4>(base + k), ib = brev<4>(base + k + half);
+            bfly_dit<k * (32 / len)>(r[ia], i[ia], r[ib], i[ib]);
+        });
+    });
+}
+
 // last stage of a decimation-in-time radix-32: (.x, .y) = (E, O) -> (E + W O, E - W O), W = W_32^K32
 template <int K32>
 __device__ __forceinline__ void bfly_dit_halves(float2 &r, float2 &i) {
@@ -263,9 +310,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     const int r_ld = r < P.R ? r : P.R - 1;        // ragged last group: recompute a valid gate, never flush it
     const long long gate_off = (long long)P.r0 + (long long)r_ld * P.stride;
     const long long run_off = (long long)P.r0 + (long long)(gg * G) * P.stride;   // first sample of the CTA's run
-    float2 acc[16];                                // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
+    float2 accS[8], accC[8];                       // per last-stage butterfly k of pass B2 (bfly_power)
 #pragma unroll
-    for (int j = 0; j < 16; j++) acc[j] = make_float2(0.f, 0.f);
+    for (int j = 0; j < 8; j++) accS[j] = accC[j] = make_float2(0.f, 0.f);
     for (int p = p_lo; p < p_hi; p++) {
         const bool has_next = p + 1 < p_hi || more_tiles;
         const int p_next = p + 1 < p_hi ? p + 1 : 0;
@@ -345,15 +392,17 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             mbar_wait(free_mbar, free_parity);
             free_parity ^= 1u;
         }
-        auto store_y = [&](auto jj_, auto f_) {                  // y_{f}[t_lo] -> region of pass-B warp (g, f)
+        auto store_y = [&](auto jj_, auto f_, float2 yr, float2 yi) {   // y_{f}[t_lo] -> region of pass-B warp (g, f)
             constexpr int jj = decltype(jj_)::value, f = decltype(f_)::value;
-            constexpr int ph = jj * RA + brev<LOGRA>(f);
             const int ap = wa + RA * jj;
             float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
-            dst[0] = xr[ph];
-            dst[32] = xi[ph];
+            dst[0] = yr;
+            dst[32] = yi;
         };
-        sfor<0, NJ>([&](auto jj_) { store_y(jj_, std::integral_constant<int, 0>{}); });
+        sfor<0, NJ>([&](auto jj_) {
+            constexpr int jj = decltype(jj_)::value;
+            store_y(jj_, std::integral_constant<int, 0>{}, xr[jj * RA], xi[jj * RA]);
+        });
         sfor<0, (NE + 1) / 2>([&](auto g_) {
             constexpr int gi = decltype(g_)::value;
             float(&cur)[8] = (gi & 1) ? two : twe;
@@ -367,10 +416,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                     constexpr int jj = e / (RA - 1), f = e % (RA - 1) + 1;
                     constexpr int ph = jj * RA + brev<LOGRA>(f);
                     const float2 wr = make_float2(cur[4 * k], cur[4 * k + 1]), wi = make_float2(cur[4 * k + 2], cur[4 * k + 3]);
-                    const float2 yr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
-                    const float2 yi = pfma(xr[ph], wi, pmul(xi[ph], wr));
-                    xr[ph] = yr; xi[ph] = yi;
-                    store_y(std::integral_constant<int, jj>{}, std::integral_constant<int, f>{});
+                    store_y(std::integral_constant<int, jj>{}, std::integral_constant<int, f>{},
+                            pfma(xr[ph], wr, pneg(pmul(xi[ph], wi))), pfma(xr[ph], wi, pmul(xi[ph], wr)));
                 }
             });
         });
@@ -427,16 +474,23 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             constexpr int bb = decltype(b_)::value;
             bfly_dif_halves<bb>(xr[bb], xi[bb]);                 // (.x, .y) -> (even e, odd e) inputs
         });
-        dft_packed<16, 0>(xr, xi);                               // (X[2 e'], X[2 e' + 1]) at brev4(e')
-#pragma unroll
-        for (int j = 0; j < 16; j++) {                           // |X|^2, accumulate (PAPER.md:79 Eq. 8, :115)
-            acc[j] = pfma(xr[j], xr[j], acc[j]);
-            acc[j] = pfma(xi[j], xi[j], acc[j]);
-        }
+        dft_packed16_head(xr, xi);
+        sfor<0, 8>([&](auto k_) {                                // last stage + |X|^2 + accumulate
+            constexpr int k = decltype(k_)::value;
+            constexpr int ia = brev<4>(k), ib = brev<4>(k + 8);
+            bfly_power<2 * k>(xr[ia], xi[ia], xr[ib], xi[ib], accS[k], accC[k]);
+        });
     }
     // ---- flush: S_dev[r][q][f_hi = wa][e][c = lane]; other CTAs may hold the rest of this tile's IPPs
     if (r < P.R) {
         float *Srow = P.S + (((long long)r * Q + q) * RA + wa) * 1024 + lane;
+        float2 acc[16];                            // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
+        sfor<0, 8>([&](auto k_) {
+            constexpr int k = decltype(k_)::value;
+            const float2 c2 = pmul(accC[k], make_float2(pow2w(2 * k), pow2w(2 * k)));
+            acc[brev<4>(k)] = padd(accS[k], c2);
+            acc[brev<4>(k + 8)] = psub(accS[k], c2);
+        });
         sfor<0, 16>([&](auto j_) {
             constexpr int j = decltype(j_)::value;
             constexpr int e = 2 * brev<4>(j);
