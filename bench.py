@@ -137,7 +137,7 @@ def cufft_pipeline(w, V_dev, C_dev, steps, flush):
                 v = torch.view_as_complex(V_dev[p].to(torch.float32))          # sc16 -> fp32 (a1)
             else:
                 v = V_dev[p]
-            win = v.as_strided((R, L), (w.stride, 1), w.r0)                     # overlapping windows (a2), a view
+            win = v.as_strided((R, L), (w.stride, 1), v.storage_offset() + w.r0)   # overlapping windows (a2), a view
             batch = win * C_dev[p].conj()                                       # K1 decode (a3)
             X = torch.fft.fft(batch, n=N, dim=1)                                # K2 cuFFT, zero-padded to N (a4)
             S.add_(torch.view_as_real(X).square().sum(dim=-1))                  # K3 power + accumulate (a5, a6)
