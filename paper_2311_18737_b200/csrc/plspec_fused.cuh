@@ -36,8 +36,9 @@ namespace plspec {
 
 constexpr int kRegionBytes = 16 * 65 * 8;                    // 8320
 constexpr int kFusedSmemBytes = 16 * kRegionBytes;
-// control words: stage mbarrier (8) + warp arrival counter (4) + TMEM base (4) + 16 "regions free" mbarriers
-constexpr int kStageCtlBytes = 16 + 16 * 8;
+// control words: stage mbarrier (8) + warp arrival counter (4) + TMEM base (4) + per region a "free" and a
+// "full" mbarrier
+constexpr int kStageCtlBytes = 16 + 32 * 8;
 constexpr int kStageOff = kFusedSmemBytes + kStageCtlBytes;    // voltage stage of the ST variant (16-byte aligned)
 constexpr int kSmemMax = 227 * 1024;
 constexpr int kStageMaxBytes = kSmemMax - kStageOff;
@@ -279,11 +280,19 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         for (uint32_t off = 0; off < bytes; off += 32768u)
             bulk_g2s(smem_u32(stage) + off, src - mis + off, (bytes - off) < 32768u ? (bytes - off) : 32768u, mbar);
     };
-    // free_mbar: the RA warps of gate g arrive once they have read their pass-B regions of a window (B2
-    // loads done); pass A of the next window waits on it before writing into those regions.
-    const uint32_t free_mbar = smem_u32(smem + kFusedSmemBytes + 16 + 8 * g);
+    // Region-grained hand-over instead of CTA-wide barriers.  free_mbar[region] (count 1): the pass-B warp that
+    // owns the region arrives once it has read it for the last time in a window (B2 loads done); a pass-A
+    // warp waits on it before its first store of the next window into that region.  full_mbar[region]
+    // (count RA): every pass-A warp of the gate arrives after its last store into the region; the owner waits
+    // on it before pass B1.  All warps store the regions in the same order f = 0 .. RA - 1, so the owners start
+    // pass B one after the other and the stagger carries over to the next window: in steady state nobody waits.
+    const uint32_t free_base = smem_u32(smem + kFusedSmemBytes + 16) + 8 * (g * RA);          // + 8 f
+    const uint32_t full_base = smem_u32(smem + kFusedSmemBytes + 16 + 16 * 8) + 8 * (g * RA);  // + 8 f
     if (tid == 0) {
-        for (int i = 0; i < G; i++) mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 8 * i), RA);
+        for (int i = 0; i < 16; i++) {
+            mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 8 * i), 1);
+            mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 16 * 8 + 8 * i), RA);
+        }
         if constexpr (ST) {
             mbar_init(mbar, 1);
             *cnt = 0;
@@ -295,8 +304,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
     }
     __syncthreads();
-    if (RA > 1 && lane == 0) mbar_arrive(free_mbar);                      // phase 0: the regions start out free
-    uint32_t parity = 0, free_parity = 0;
+    if (RA > 1 && lane == 0) mbar_arrive(free_base + 8 * wa);             // phase 0: the regions start out free
+    uint32_t parity = 0, free_parity = 0, full_parity = 0;
     int arrivals_target = 15;                                              // 16 warps per IPP, 0-based last
 
     int left = (int)(i1 - i0);                     // items still to do, this one included
@@ -385,19 +394,18 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             }
             arrivals_target += 16;
         }
-        // the gate's warps are done reading their regions for the previous window
-        if constexpr (RA == 1) {
-            __syncwarp();
-        } else {
-            mbar_wait(free_mbar, free_parity);
-            free_parity ^= 1u;
-        }
+        if constexpr (RA == 1) __syncwarp();
         auto store_y = [&](auto jj_, auto f_, float2 yr, float2 yi) {   // y_{f}[t_lo] -> region of pass-B warp (g, f)
             constexpr int jj = decltype(jj_)::value, f = decltype(f_)::value;
             const int ap = wa + RA * jj;
             float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
+            if constexpr (RA > 1 && jj == 0) mbar_wait(free_base + 8 * f, free_parity);   // owner has read the previous window
             dst[0] = yr;
             dst[32] = yi;
+            if constexpr (RA > 1 && jj == NJ - 1) {                      // this warp's last store into region f
+                __syncwarp();
+                if (lane == 0) mbar_arrive(full_base + 8 * f);
+            }
         };
         sfor<0, NJ>([&](auto jj_) {
             constexpr int jj = decltype(jj_)::value;
@@ -421,7 +429,13 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 }
             });
         });
-        if constexpr (RA == 1) __syncwarp(); else named_bar_sync(1 + g, RA * 32);
+        if constexpr (RA == 1) {
+            __syncwarp();
+        } else {
+            free_parity ^= 1u;
+            mbar_wait(full_base + 8 * wa, full_parity);                  // every pass-A warp has filled this warp's region
+            full_parity ^= 1u;
+        }
 
         // ---- pass B1: lane = b; decimation-in-time radix-32 over a; .x = even a, .y = odd a
         {
@@ -468,7 +482,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
         if constexpr (RA > 1) {                                  // this warp's region may be overwritten again
             __syncwarp();
-            if (lane == 0) mbar_arrive(free_mbar);
+            if (lane == 0) mbar_arrive(free_base + 8 * wa);
         }
         sfor<0, 16>([&](auto b_) {
             constexpr int bb = decltype(b_)::value;
