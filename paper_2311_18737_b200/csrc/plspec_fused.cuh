@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     auto resid_of = [&](int t) { return Q == 1 ? 0 : t / P.n_groups; };
 
     // ---- twiddles live in tensor memory: every thread re-reads only constants it wrote itself
-    //   columns [4 e, 4 e + 4), e = jj (RA - 1) + f - 1:  pass A -> B1, W_Nk^{t_lo f} for the thread's two t_lo
+    //   columns [4 e, 4 e + 4), e = (f - 1) NJ + jj:      pass A -> B1, W_Nk^{t_lo f} for the thread's two t_lo
     //   columns [64 + 4 c', ..):                           B1 -> B2,   W_1024^{b c'}, W_1024^{b (c' + 16)}, b = lane
     uint32_t *const tm_slot = reinterpret_cast<uint32_t *>(smem + kFusedSmemBytes + 12);
     if (warp == 0) tmem_alloc_512(smem_u32(tm_slot));
@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             constexpr int f = decltype(f_)::value;
             const float2 wr = __ldg(P.twA + ((ap * RA + f) * 2 + 0) * 32 + lane);
             const float2 wi = __ldg(P.twA + ((ap * RA + f) * 2 + 1) * 32 + lane);
-            tmem_st4(tm + 4 * (jj * (RA - 1) + f - 1), wr.x, wr.y, wi.x, wi.y);
+            tmem_st4(tm + 4 * ((f - 1) * NJ + jj), wr.x, wr.y, wi.x, wi.y);
         });
     });
     sfor<0, 16>([&](auto c_) {
@@ -421,7 +421,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 constexpr int k = decltype(k_)::value;
                 constexpr int e = gi * 2 + k;
                 if constexpr (e < NE) {
-                    constexpr int jj = e / (RA - 1), f = e % (RA - 1) + 1;
+                    constexpr int jj = e % NJ, f = e / NJ + 1;
                     constexpr int ph = jj * RA + brev<LOGRA>(f);
                     const float2 wr = make_float2(cur[4 * k], cur[4 * k + 1]), wi = make_float2(cur[4 * k + 2], cur[4 * k + 3]);
                     store_y(std::integral_constant<int, jj>{}, std::integral_constant<int, f>{},
