@@ -553,6 +553,7 @@ int plspec_finalize(plspec_handle h, float *S_out) {
     cudaStream_t st = h->last_stream;
     const size_t total = (size_t)h->R * (size_t)h->N;
     const float *src = h->S;
+    bool zeroed = false;
     if (h->Q > 1 || h->kind == 2) {                      // S_dev is not in natural bin order
         float *dst = S_out;
         if (!out_dev) {
@@ -562,18 +563,22 @@ int plspec_finalize(plspec_handle h, float *S_out) {
             }
             dst = h->S_tmp;
         }
-        unpermute_kernel<<<h->n_sm * 8, 256, 0, st>>>(h->S, dst, h->Q, h->Nk, h->kind == 2 ? h->RA : 0,
-                                                       (long long)total);
+        // one pass: transposition to natural bin order + zeroing of the accumulators
+        const int RAe = h->kind == 2 ? h->RA : 1, NC = h->kind == 2 ? 1024 : h->Nk, M = h->Q * RAe;
+        int TC = 4096 / M < NC ? 4096 / M : NC;
+        finalize_kernel<<<dim3((unsigned)h->R, (unsigned)(NC / TC)), 256, (size_t)TC * (M + 1) * sizeof(float), st>>>(
+            h->S, dst, ilog2(h->Q), ilog2(RAe), NC, TC);
         PL_CUDA(h, cudaGetLastError());
         h->stats.kernel_launches++;
         src = dst;
+        zeroed = true;
     }
     if (src != S_out) {
         PL_CUDA(h, cudaMemcpyAsync(S_out, src, total * sizeof(float),
                                    out_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
         if (!out_dev) h->stats.d2h_bytes += (long long)(total * sizeof(float));
     }
-    PL_CUDA(h, cudaMemsetAsync(h->S, 0, total * sizeof(float), st));
+    if (!zeroed) PL_CUDA(h, cudaMemsetAsync(h->S, 0, total * sizeof(float), st));
     PL_CUDA(h, cudaStreamSynchronize(st));
     h->have_work = false;
     return PLSPEC_OK;

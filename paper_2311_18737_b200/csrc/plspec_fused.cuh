@@ -28,7 +28,7 @@
 // Both are free of bank conflicts (the 65 pitch spreads the 4-byte transposed stores over all banks).
 //
 // S_dev layout written by this kernel: [r][q][f_hi][e][c]  (c = lane: every flush is 128 B per warp);
-// unpermute_kernel restores natural bin order at finalize.
+// finalize_kernel restores natural bin order at finalize.
 #pragma once
 #include "plspec_common.cuh"
 
@@ -519,22 +519,43 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     if (warp == 0) tmem_dealloc_512(tm_base);
 }
 
-// S_out[r][q + Q (f_hi + RA (c + 32 e))] = S_dev[r][q][f_hi][e][c]   (fused layout), or
-// S_out[r][q + Q k]                      = S_dev[r][q][k]             (generic layout, RA = 0)
-__global__ void unpermute_kernel(const float *__restrict__ Sdev, float *__restrict__ Sout, int Q, int Nk, int RA,
-                                 long long total) {
-    const int N = Q * Nk;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
-         i += (long long)gridDim.x * blockDim.x) {
-        const long long r = i / N;
-        const int f = (int)(i - r * N);
-        const int q = f % Q, k = f / Q;
-        int src = k;
-        if (RA > 0) {
-            const int f_hi = k % RA, k_lo = k / RA;
-            src = (f_hi * 32 + (k_lo >> 5)) * 32 + (k_lo & 31);
+// Finalize: natural bin order out, accumulators zeroed, one pass over S.  Per gate S_dev is an
+// M x NC matrix, row j_in = q RAe + f_hi (M = Q RAe rows; fused layout: RAe = RA, NC = 1024; generic layout:
+// RAe = 1, NC = Nk), and S_out[r][(f_hi Q + q) + M col] = S_dev[r][j_in][col]: a transposition.  A block moves a tile
+// of all M rows x TC columns through shared memory (pitch M + 1), so both the reads and the writes are
+// contiguous runs, and writes zeros back over what it has read.
+__global__ void __launch_bounds__(256) finalize_kernel(float *__restrict__ Sdev, float *__restrict__ Sout, int log2Q,
+                                                       int log2RAe, int NC, int TC) {
+    extern __shared__ float tile[];
+    const int log2M = log2Q + log2RAe, M = 1 << log2M, Q = 1 << log2Q, RAe = 1 << log2RAe;
+    const long long gate = blockIdx.x;
+    const int c0 = blockIdx.y * TC;
+    float *X = Sdev + gate * (long long)M * NC;
+    float *Y = Sout + gate * (long long)M * NC + (long long)c0 * M;
+    const int n = M * TC;
+    int log2TC = 0;
+    while ((1 << log2TC) < TC) log2TC++;
+    auto src_of = [&](int i) { return X + (long long)(i >> log2TC) * NC + c0 + (i & (TC - 1)); };
+    for (int i0 = threadIdx.x; i0 < n; i0 += 8 * blockDim.x) {          // eight independent loads in flight per thread
+        float v[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            const int i = i0 + u * blockDim.x;
+            v[u] = i < n ? __ldcs(src_of(i)) : 0.0f;
         }
-        Sout[i] = Sdev[(r * Q + q) * Nk + src];
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            const int i = i0 + u * blockDim.x;
+            const int j = i >> log2TC, c = i & (TC - 1);
+            const int q = j >> log2RAe, f_hi = j & (RAe - 1);
+            if (i < n) tile[c * (M + 1) + f_hi * Q + q] = v[u];
+        }
+    }
+    __syncthreads();
+    // zeros go back only now: a store to a line whose load is still in flight stalls the memory pipeline
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        Y[i] = tile[i + (i >> log2M)];
+        *src_of(i) = 0.0f;
     }
 }
 
