@@ -280,17 +280,18 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         for (uint32_t off = 0; off < bytes; off += 32768u)
             bulk_g2s(smem_u32(stage) + off, src - mis + off, (bytes - off) < 32768u ? (bytes - off) : 32768u, mbar);
     };
-    // Region-grained hand-over instead of CTA-wide barriers.  free_mbar[region] (count 1): the pass-B warp that
-    // owns the region arrives once it has read it for the last time in a window (B2 loads done); a pass-A
-    // warp waits on it before its first store of the next window into that region.  full_mbar[region]
-    // (count RA): every pass-A warp of the gate arrives after its last store into the region; the owner waits
-    // on it before pass B1.  All warps store the regions in the same order f = 0 .. RA - 1, so the owners start
-    // pass B one after the other and the stagger carries over to the next window: in steady state nobody waits.
-    const uint32_t free_base = smem_u32(smem + kFusedSmemBytes + 16) + 8 * (g * RA);          // + 8 f
+    // Hand-over of the exchange regions without CTA-wide barriers.  full_mbar[region] (count RA): every pass-A
+    // warp of the gate arrives after its last store into the region; the region's owner waits on it before
+    // pass B1.  All warps store the regions in the same order f = 0 .. RA - 1, so the owners start pass B one
+    // after the other and the stagger carries over to the next window: in steady state nobody waits.
+    // free_mbar[gate] (count RA): each owner arrives once it has read its region for the last time in a window
+    // (B2 loads done); a pass-A warp waits on it before its first store of the next window (by then the last
+    // owner is long past that point, and one probe per window is cheaper than one per region).
+    const uint32_t free_base = smem_u32(smem + kFusedSmemBytes + 16) + 8 * (g * RA);
     const uint32_t full_base = smem_u32(smem + kFusedSmemBytes + 16 + 16 * 8) + 8 * (g * RA);  // + 8 f
     if (tid == 0) {
         for (int i = 0; i < 16; i++) {
-            mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 8 * i), 1);
+            mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 8 * i), RA);
             mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 16 * 8 + 8 * i), RA);
         }
         if constexpr (ST) {
@@ -304,7 +305,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
     }
     __syncthreads();
-    if (RA > 1 && lane == 0) mbar_arrive(free_base + 8 * wa);             // phase 0: the regions start out free
+    if (RA > 1 && lane == 0) mbar_arrive(free_base);                      // phase 0: the regions start out free
     uint32_t parity = 0, free_parity = 0, full_parity = 0;
     int arrivals_target = 15;                                              // 16 warps per IPP, 0-based last
 
@@ -395,11 +396,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             arrivals_target += 16;
         }
         if constexpr (RA == 1) __syncwarp();
+        else mbar_wait(free_base, free_parity);                          // every owner has read the previous window
         auto store_y = [&](auto jj_, auto f_, float2 yr, float2 yi) {   // y_{f}[t_lo] -> region of pass-B warp (g, f)
             constexpr int jj = decltype(jj_)::value, f = decltype(f_)::value;
             const int ap = wa + RA * jj;
             float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
-            if constexpr (RA > 1 && jj == 0) mbar_wait(free_base + 8 * f, free_parity);   // owner has read the previous window
             dst[0] = yr;
             dst[32] = yi;
             if constexpr (RA > 1 && jj == NJ - 1) {                      // this warp's last store into region f
@@ -482,7 +483,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
         if constexpr (RA > 1) {                                  // this warp's region may be overwritten again
             __syncwarp();
-            if (lane == 0) mbar_arrive(free_base + 8 * wa);
+            if (lane == 0) mbar_arrive(free_base);
         }
         sfor<0, 16>([&](auto b_) {
             constexpr int bb = decltype(b_)::value;
