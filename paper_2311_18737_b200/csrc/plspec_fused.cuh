@@ -216,6 +216,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     constexpr int NJ = 16 / RA;            // a' values per thread in pass A
     constexpr int G = 16 / RA;             // gates per CTA
     constexpr int LOGRA = ilog2(RA);
+    constexpr int FG = RA == 16 ? 4 : 1;   // regions per "full" mbarrier (measured: 4 at RA = 16, 1 below)
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = warp / RA, wa = warp % RA;       // pass A: warp `wa` of gate g;  pass B: (gate g, f_hi = wa)
@@ -283,7 +284,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     // Hand-over of the exchange regions without CTA-wide barriers.  full_mbar[region] (count RA): every pass-A
     // warp of the gate arrives after its last store into the region; the region's owner waits on it before
     // pass B1.  All warps store the regions in the same order f = 0 .. RA - 1, so the owners start pass B one
-    // after the other and the stagger carries over to the next window: in steady state nobody waits.
+    // after the other and the stagger carries over to the next window: in steady state nobody waits.  At
+    // RA = 16 four neighbouring regions share one mbarrier (4 arrivals per warp and window instead of 16).
     // free_mbar[gate] (count RA): each owner arrives once it has read its region for the last time in a window
     // (B2 loads done); a pass-A warp waits on it before its first store of the next window (by then the last
     // owner is long past that point, and one probe per window is cheaper than one per region).
@@ -403,9 +405,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
             dst[0] = yr;
             dst[32] = yi;
-            if constexpr (RA > 1 && jj == NJ - 1) {                      // this warp's last store into region f
+            if constexpr (RA > 1 && jj == NJ - 1 && (f % FG == FG - 1 || f == RA - 1)) {   // last store into the regions of group f / FG
                 __syncwarp();
-                if (lane == 0) mbar_arrive(full_base + 8 * f);
+                if (lane == 0) mbar_arrive(full_base + 8 * (f / FG));
             }
         };
         sfor<0, NJ>([&](auto jj_) {
@@ -434,7 +436,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             __syncwarp();
         } else {
             free_parity ^= 1u;
-            mbar_wait(full_base + 8 * wa, full_parity);                  // every pass-A warp has filled this warp's region
+            mbar_wait(full_base + 8 * (wa / FG), full_parity);                  // every pass-A warp has filled this warp's region
             full_parity ^= 1u;
         }
 
