@@ -311,6 +311,24 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     uint32_t parity = 0, free_parity = 0, full_parity = 0;
     int arrivals_target = 15;                                              // 16 warps per IPP, 0-based last
 
+    // PF: the raw samples (one 32-bit word each) and the code word of the NEXT window are fetched while the last
+    // butterfly stage of the current one retires its registers, so no warp sits on L2 latency at the top of a window
+    constexpr bool PF = RA == 16 && Q == 1 && DT == DT_SC16 && !ST;
+    uint32_t raw[PF ? 32 : 1], cw_pf = 0;
+    auto pf_base = [&](int t, int pp) {            // this thread's first sample of (tile t, IPP pp)
+        const int rr = group_of(t) * G + g;
+        const long long off = (long long)P.r0 + (long long)(rr < P.R ? rr : P.R - 1) * P.stride;
+        return reinterpret_cast<const uint32_t *>(P.V) + (long long)pp * P.v_pitch + off + 64 * wa + lane;
+    };
+    if constexpr (PF) {
+        if (bpsk) {
+            const uint32_t *b = pf_base(tile0, p0);
+#pragma unroll
+            for (int i = 0; i < 32; i++) raw[i] = __ldg(b + (i >> 1) * 1024 + (i & 1) * 32);
+            cw_pf = __ldg(P.Cbits + (long long)p0 * 512 + wa * 32 + lane);
+        }
+    }
+
     int left = (int)(i1 - i0);                     // items still to do, this one included
     int p_lo = p0;
     for (int tile = tile0; left > 0; tile++, p_lo = 0) {                   // the tiles this CTA's run touches
@@ -341,7 +359,15 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
         float2 xr[16], xi[16];
         // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
-        if (bpsk) {
+        if (PF && bpsk) {
+            if constexpr (PF) {
+                sfor<0, RA>([&](auto th_) {
+                    constexpr int th = decltype(th_)::value;
+                    sc16_pair_to_f32(raw[2 * th], raw[2 * th + 1], bit_mask<2 * th>(cw_pf), bit_mask<2 * th + 1>(cw_pf),
+                                     xr[th], xi[th]);
+                });
+            }
+        } else if (bpsk) {
             sfor<0, NJ>([&](auto jj_) {
                 constexpr int jj = decltype(jj_)::value;
                 const int ap = wa + RA * jj;
@@ -492,10 +518,21 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             bfly_dif_halves<bb>(xr[bb], xi[bb]);                 // (.x, .y) -> (even e, odd e) inputs
         });
         dft_packed16_head(xr, xi);
+        const uint32_t *pf_next = nullptr;
         sfor<0, 8>([&](auto k_) {                                // last stage + |X|^2 + accumulate
             constexpr int k = decltype(k_)::value;
             constexpr int ia = brev<4>(k), ib = brev<4>(k + 8);
             bfly_power<2 * k>(xr[ia], xi[ia], xr[ib], xi[ib], accS[k], accC[k]);
+            if constexpr (PF) {                                  // eight registers just died: four words of the next window
+                // unconditional (the last window fetches its own samples again): every word is redefined in every
+                // window, so none of them stays live through passes A and B
+                if constexpr (k == 0) pf_next = has_next ? pf_base(tile_next, p_next) : pf_base(tile, p);
+#pragma unroll
+                for (int i = 4 * k; i < 4 * k + 4; i++) raw[i] = __ldg(pf_next + (i >> 1) * 1024 + (i & 1) * 32);
+                if constexpr (k == 7) {
+                    if (bpsk) cw_pf = __ldg(P.Cbits + (long long)(has_next ? p_next : p) * 512 + wa * 32 + lane);
+                }
+            }
         });
     }
     // ---- flush: S_dev[r][q][f_hi = wa][e][c = lane]; other CTAs may hold the rest of this tile's IPPs
