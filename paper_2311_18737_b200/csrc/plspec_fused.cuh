@@ -313,18 +313,28 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
 
     // PF: the raw samples (one 32-bit word each) and the code word of the NEXT window are fetched while the last
     // butterfly stage of the current one retires its registers, so no warp sits on L2 latency at the top of a window
-    constexpr bool PF = RA == 16 && Q == 1 && DT == DT_SC16 && !ST;
-    uint32_t raw[PF ? 32 : 1], cw_pf = 0;
+    constexpr bool PF = RA == 16 && Q == 1 && !ST;
+    constexpr int WPS = DT == DT_SC16 ? 1 : 2;     // 32-bit words per sample
+    uint32_t raw[PF ? 32 * WPS : 1], cw_pf = 0;
     auto pf_base = [&](int t, int pp) {            // this thread's first sample of (tile t, IPP pp)
         const int rr = group_of(t) * G + g;
         const long long off = (long long)P.r0 + (long long)(rr < P.R ? rr : P.R - 1) * P.stride;
-        return reinterpret_cast<const uint32_t *>(P.V) + (long long)pp * P.v_pitch + off + 64 * wa + lane;
+        return reinterpret_cast<const uint32_t *>(P.V) + ((long long)pp * P.v_pitch + off + 64 * wa + lane) * WPS;
+    };
+    auto pf_load = [&](const uint32_t *b, auto i_) {   // sample i = 2 t_hi + o of the thread's window
+        constexpr int i = decltype(i_)::value;
+        if constexpr (DT == DT_SC16) {
+            raw[i] = __ldg(b + (i >> 1) * 1024 + (i & 1) * 32);
+        } else {
+            const uint2 v = __ldg(reinterpret_cast<const uint2 *>(b) + (i >> 1) * 1024 + (i & 1) * 32);
+            raw[2 * i] = v.x;
+            raw[2 * i + 1] = v.y;
+        }
     };
     if constexpr (PF) {
         if (bpsk) {
             const uint32_t *b = pf_base(tile0, p0);
-#pragma unroll
-            for (int i = 0; i < 32; i++) raw[i] = __ldg(b + (i >> 1) * 1024 + (i & 1) * 32);
+            sfor<0, 32>([&](auto i_) { pf_load(b, i_); });
             cw_pf = __ldg(P.Cbits + (long long)p0 * 512 + wa * 32 + lane);
         }
     }
@@ -363,8 +373,15 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             if constexpr (PF) {
                 sfor<0, RA>([&](auto th_) {
                     constexpr int th = decltype(th_)::value;
-                    sc16_pair_to_f32(raw[2 * th], raw[2 * th + 1], bit_mask<2 * th>(cw_pf), bit_mask<2 * th + 1>(cw_pf),
-                                     xr[th], xi[th]);
+                    const uint32_t m0 = bit_mask<2 * th>(cw_pf), m1 = bit_mask<2 * th + 1>(cw_pf);
+                    if constexpr (DT == DT_SC16) {
+                        sc16_pair_to_f32(raw[2 * th], raw[2 * th + 1], m0, m1, xr[th], xi[th]);
+                    } else {                                     // +-1 code: flip the sign bits
+                        xr[th] = make_float2(__uint_as_float(raw[4 * th] ^ (m0 & 0x80000000u)),
+                                             __uint_as_float(raw[4 * th + 2] ^ (m1 & 0x80000000u)));
+                        xi[th] = make_float2(__uint_as_float(raw[4 * th + 1] ^ (m0 & 0x80000000u)),
+                                             __uint_as_float(raw[4 * th + 3] ^ (m1 & 0x80000000u)));
+                    }
                 });
             }
         } else if (bpsk) {
@@ -527,8 +544,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 // unconditional (the last window fetches its own samples again): every word is redefined in every
                 // window, so none of them stays live through passes A and B
                 if constexpr (k == 0) pf_next = has_next ? pf_base(tile_next, p_next) : pf_base(tile, p);
-#pragma unroll
-                for (int i = 4 * k; i < 4 * k + 4; i++) raw[i] = __ldg(pf_next + (i >> 1) * 1024 + (i & 1) * 32);
+                sfor<4 * k, 4 * k + 4>([&](auto i_) { pf_load(pf_next, i_); });
                 if constexpr (k == 7) {
                     if (bpsk) cw_pf = __ldg(P.Cbits + (long long)(has_next ? p_next : p) * 512 + wa * 32 + lane);
                 }
