@@ -57,6 +57,7 @@ struct plspec_ctx {
     uint32_t *cbits = nullptr;       // packed code signs of the launch in flight (BPSK fast path)
     long long cbits_words = 0;
     int *not_bpsk = nullptr;         // device flag written by pack_codes_kernel
+    int epoch = 0;                   // number of the last code pre-pass
     // host pipeline
     cudaStream_t copy_stream = nullptr;
     Slot slot[kSlots];
@@ -186,7 +187,7 @@ int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long
     P.n_ipp = n_ipp;
     P.n_chunks = pick_chunks(h, n_ipp);
     P.use_atomic = P.n_chunks > 1 ? 1 : 0;
-    P.Cbits = nullptr; P.not_bpsk = nullptr;
+    P.Cbits = nullptr; P.not_bpsk = nullptr; P.epoch = 1;
     if (h->kind == 2 && h->opt_bpsk && h->L == h->N) {
         // code pre-pass: pack the signs of real +-1 codes (1 bit / sample instead of 8 bytes); the fused
         // kernel falls back to the general complex decode when the flag says the codes are anything else
@@ -200,8 +201,9 @@ int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long
             }
             h->cbits_words = words;
         }
-        PL_CUDA(h, cudaMemsetAsync(h->not_bpsk, 0, sizeof(int), stream));
-        pack_codes_kernel<<<(unsigned)((words + 255) / 256), 256, 0, stream>>>(dC, h->cbits, h->not_bpsk, h->L, h->Nk,
+        h->epoch = h->epoch == 0x7fffffff ? 1 : h->epoch + 1;
+        P.epoch = h->epoch;
+        pack_codes_kernel<<<(unsigned)((words + 255) / 256), 256, 0, stream>>>(dC, h->cbits, h->not_bpsk, h->epoch, h->L, h->Nk,
                                                                               h->RA, h->Q, words);
         PL_CUDA(h, cudaGetLastError());
         h->stats.kernel_launches++;
@@ -260,7 +262,7 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
         P.V = (const char *)dV + (size_t)p0 * (size_t)v_pitch * esz;
         P.C = dC + (size_t)p0 * h->L;
         P.S = h->S; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
-        P.Cbits = nullptr; P.not_bpsk = nullptr;
+        P.Cbits = nullptr; P.not_bpsk = nullptr; P.epoch = 1;
         P.v_pitch = v_pitch;
         P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
         P.L = h->L; P.R = h->R; P.r0 = r0; P.stride = h->stride;
@@ -343,8 +345,12 @@ int ensure_slots(plspec_ctx *h, int batch) {
 // on the copy stream, overlapped with the kernels of earlier batches (PAPER.md:149 item 2).
 int accumulate_from_host(plspec_ctx *h, const void *V, const void *C, int n_ipp, cudaStream_t stream) {
     const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
-    int batch = h->opt_batch > 0 ? h->opt_batch : (n_ipp + 7) / 8;
     const size_t per_ipp = (size_t)h->span * esz + (size_t)h->L * sizeof(float2);
+    // auto: eight batches per call, but none below ~4 MB (each batch pays the launches' fixed cost once)
+    int batch = (n_ipp + 7) / 8;
+    const int min_batch = (int)(((size_t)4 << 20) / per_ipp) + 1;
+    if (batch < min_batch) batch = min_batch;
+    if (h->opt_batch > 0) batch = h->opt_batch;
     const int cap = (int)((256u << 20) / per_ipp);        // <= 256 MiB per slot
     if (batch > cap) batch = cap;
     if (batch < 1) batch = 1;
@@ -490,6 +496,7 @@ int plspec_create(int N, int code_len, int n_ranges, int r0, int stride, int ipp
         return fail(PLSPEC_ERR_CUDA);
     }
     if (cudaMalloc((void **)&h->not_bpsk, sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_ALLOC); }
+    if (cudaMemset(h->not_bpsk, 0, sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_CUDA); }
     if ((rc = build_tables(h)) != PLSPEC_OK) return fail(rc);
     if ((rc = select_kernel(h)) != PLSPEC_OK) return fail(rc);
     *out = h;

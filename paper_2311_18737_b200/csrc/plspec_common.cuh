@@ -21,7 +21,8 @@ struct KParams {
     const float2 *twB;      // fused kernel, pass B1 -> B2: [c'][re/im][lane] pairs W_1024^{b c}
     const float2 *twN;      // [N]: exp(-2 pi i e / N), full circle
     const uint32_t *Cbits;  // fused kernel, BPSK fast path: [n_ipp][Q][512] packed code signs (or null)
-    const int    *not_bpsk; // device flag written by pack_codes_kernel: 0 = use Cbits
+    const int    *not_bpsk; // device flag written by pack_codes_kernel: != epoch -> use Cbits
+    int           epoch;    // number of this launch's code pre-pass (never 0; the flag starts at 0)
     long long     v_pitch;  // samples between successive IPP rows of V
     int N, Nk, Q, log2Nk;
     int L;                  // code_len

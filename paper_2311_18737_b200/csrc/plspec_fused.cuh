@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     });
     tmem_wait_st();
 
-    const bool bpsk = P.Cbits != nullptr && __ldg(P.not_bpsk) == 0;   // warp-uniform
+    const bool bpsk = P.Cbits != nullptr && __ldg(P.not_bpsk) != P.epoch;   // warp-uniform
 
     unsigned char *const region = smem + warp * kRegionBytes;              // this warp's pass-B region
     unsigned char *const gate_regions = smem + (g * RA) * kRegionBytes;    // regions of this gate (pass A target)

@@ -114,8 +114,9 @@ __device__ __forceinline__ void load_pair_bpsk(const VSrc &src, uint32_t cw, int
 
 // codes[n_ipp][L] (L == Q * 1024 * RA) -> bit-packed words in the fused kernel's pass-A thread order:
 // Cbits[p][j][ap * 32 + lane], bit (th * 2 + o) <-> t = j Nk + th 1024 + 64 ap + lane + 32 o.
-// *not_bpsk is set to 1 if any sample is not exactly +-1 + 0j (the fused kernel then decodes generally).
-__global__ void pack_codes_kernel(const float2 *__restrict__ C, uint32_t *__restrict__ Cbits, int *not_bpsk,
+// *not_bpsk is set to this pre-pass's number `epoch` if any sample is not exactly +-1 + 0j (the fused kernel
+// then decodes generally); a flag left by an earlier pre-pass never equals it, so nothing has to be cleared.
+__global__ void pack_codes_kernel(const float2 *__restrict__ C, uint32_t *__restrict__ Cbits, int *not_bpsk, int epoch,
                                   int L, int Nk, int RA, int Q, long long total_words) {
     const long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= total_words) return;
@@ -133,7 +134,7 @@ __global__ void pack_codes_kernel(const float2 *__restrict__ C, uint32_t *__rest
             bits |= (c.x < 0.f ? 1u : 0u) << (th * 2 + o);
         }
     Cbits[w] = bits;
-    if (!ok) atomicOr(not_bpsk, 1);
+    if (!ok) *not_bpsk = epoch;
 }
 
 // ------------------------------------------------------------------------------------------
