@@ -291,3 +291,27 @@ def test_cfg3_full_size_sampled_gates():
     for g in range(0, w.n_ranges, 37):
         energy = (cs[:, g + w.code_len] - cs[:, g]).sum()
         assert abs(S_gpu[g].astype(np.float64).sum() / (w.N * energy) - 1.0) < 1e-5
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "paper"])
+def test_other_workloads_full_size_sampled_gates(name):
+    """The other bench workloads at full size, in the launch configuration bench.py times (staged 4 / 2 gates per
+    CTA, split path above 16384, stride 25): oracle on sampled gates, Parseval on a gate grid."""
+    w = synth.CONFIGS[name]
+    V, C = synth.make_inputs(w)
+    S_gpu, stats = run_gpu(w, V, C)
+    R = w.n_ranges
+    gates = sorted({0, 1, 2, 3, 4, R // 3, R // 2, R - 2, R - 1})
+    for g in gates:
+        ref = oracle.spectra(V, C, N=w.N, n_ranges=1, r0=w.r0 + g * w.stride, stride=1)
+        m = gate_metric(S_gpu[g:g + 1], ref)
+        assert m.max() <= TOL, f"{name} gate {g}: {m.max():.3e}"
+    if w.dtype == synth.SC16:
+        Vf = V[..., 0].astype(np.float64) ** 2 + V[..., 1].astype(np.float64) ** 2
+    else:
+        Vf = V.real.astype(np.float64) ** 2 + V.imag.astype(np.float64) ** 2
+    cs = np.concatenate([np.zeros((w.n_ipp, 1)), np.cumsum(Vf, axis=1)], axis=1)
+    for g in range(0, R, 41):
+        off = w.r0 + g * w.stride
+        energy = (cs[:, off + w.code_len] - cs[:, off]).sum()
+        assert abs(S_gpu[g].astype(np.float64).sum() / (w.N * energy) - 1.0) < 1e-5, f"{name} gate {g}"
