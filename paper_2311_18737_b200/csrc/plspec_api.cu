@@ -175,6 +175,24 @@ int pick_chunks(const plspec_ctx *h, int n_ipp) {
 int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp,
                  cudaStream_t stream);
 
+// The fused kernel is launched with programmatic stream serialisation: its prologue (TMEM allocation, twiddle
+// tables) overlaps the tail of whatever precedes it in the stream; it calls griddepcontrol.wait before it reads
+// or writes anything earlier work produces.
+cudaError_t launch_fused(const void *func, unsigned grid, unsigned block, void **args, size_t smem, cudaStream_t stream,
+                         bool pdl) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelExC(&cfg, func, args);
+}
+
 int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0,
                       int n_ipp, cudaStream_t stream) {
     if (h->kind == 2 && h->split) return launch_split(h, dV, dC, v_pitch, r0, n_ipp, stream);
@@ -225,7 +243,7 @@ int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long
     h->stats.ipp_chunks_last = P.n_chunks;
     if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
     void *args[] = {&P};
-    PL_CUDA(h, cudaLaunchKernel(h->kfunc, dim3((unsigned)tiles), dim3((unsigned)h->block), args, h->smem, stream));
+    PL_CUDA(h, launch_fused(h->kfunc, (unsigned)tiles, (unsigned)h->block, args, h->smem, stream, h->kind == 2));
     h->stats.kernel_launches++;
     return PLSPEC_OK;
 }
@@ -300,8 +318,8 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
         h->stats.ipp_chunks_last = F.n_chunks;
         if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
         void *args[] = {&F};
-        PL_CUDA(h, cudaLaunchKernel(h->kfunc_split, dim3((unsigned)tiles), dim3((unsigned)kFusedThreads), args,
-                                    (size_t)kStageOff, stream));
+        PL_CUDA(h, launch_fused(h->kfunc_split, (unsigned)tiles, (unsigned)kFusedThreads, args, (size_t)kStageOff, stream,
+                                true));
         h->stats.kernel_launches++;
     }
     return PLSPEC_OK;

@@ -164,6 +164,12 @@ __device__ __forceinline__ void tmem_wait_ld16(float (&v)[16]) {
                    "+f"(v[8]), "+f"(v[9]), "+f"(v[10]), "+f"(v[11]), "+f"(v[12]), "+f"(v[13]), "+f"(v[14]), "+f"(v[15]));
 }
 
+// Programmatic dependent launch: a kernel launched with the stream-serialisation attribute may start while
+// its predecessor in the stream is still running; it must not touch anything the predecessor (or any earlier
+// work) writes before pdl_wait() returns.  Both are no-ops in a plain launch.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // compile-time loop
 template <int B, int E, class F>
 __device__ __forceinline__ void sfor(F &&f) {

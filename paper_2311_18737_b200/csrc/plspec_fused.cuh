@@ -260,6 +260,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     });
     tmem_wait_st();
 
+    pdl_wait();   // everything above (TMEM, twiddles) may overlap the code pre-pass / decode pre-pass before us
     const bool bpsk = P.Cbits != nullptr && __ldg(P.not_bpsk) != P.epoch;   // warp-uniform
 
     unsigned char *const region = smem + warp * kRegionBytes;              // this warp's pass-B region

@@ -118,6 +118,7 @@ __device__ __forceinline__ void load_pair_bpsk(const VSrc &src, uint32_t cw, int
 // then decodes generally); a flag left by an earlier pre-pass never equals it, so nothing has to be cleared.
 __global__ void pack_codes_kernel(const float2 *__restrict__ C, uint32_t *__restrict__ Cbits, int *not_bpsk, int epoch,
                                   int L, int Nk, int RA, int Q, long long total_words) {
+    pdl_launch_dependents();                       // the fused kernel's prologue may start now
     const long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= total_words) return;
     const int lane = (int)(w & 31), ap = (int)((w >> 5) & 15);
