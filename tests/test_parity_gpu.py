@@ -315,3 +315,20 @@ def test_other_workloads_full_size_sampled_gates(name):
         off = w.r0 + g * w.stride
         energy = (cs[:, off + w.code_len] - cs[:, off]).sum()
         assert abs(S_gpu[g].astype(np.float64).sum() / (w.N * energy) - 1.0) < 1e-5, f"{name} gate {g}"
+
+
+@pytest.mark.parametrize("N,dtype", [(16384, synth.SC16), (16384, synth.CF32), (8192, synth.SC16), (4096, synth.CF32)])
+def test_repeated_runs_agree(N, dtype):
+    """The exchange regions are handed over by mbarriers alone (no CTA-wide barrier): a hazard there would show
+    up as run-to-run differences.  25 integrations of the same input, each compared with the oracle; between
+    runs only the order of the (at most three) partial sums that meet in one accumulator may differ."""
+    w, V, C = random_case(N, N, 310, 2, 3, 9, dtype, complex_code=False)
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    first = None
+    for _ in range(25):
+        S_gpu, _ = run_gpu(w, V, C)
+        assert gate_metric(S_gpu, S_ref).max() <= TOL
+        if first is None:
+            first = S_gpu
+        else:
+            assert np.abs(S_gpu - first).max() <= 1e-6 * S_ref.mean()
