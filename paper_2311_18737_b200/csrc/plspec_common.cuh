@@ -151,19 +151,6 @@ __device__ __forceinline__ void tmem_wait_ld8(float (&v)[8]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;"
                  : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]));
 }
-// 16 consecutive columns -> v[0..15]; the values may be used only after tmem_wait_ld16(v)
-__device__ __forceinline__ void tmem_ld16(uint32_t a, float (&v)[16]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]),
-                   "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
-                 : "r"(a));
-}
-__device__ __forceinline__ void tmem_wait_ld16(float (&v)[16]) {
-    asm volatile("tcgen05.wait::ld.sync.aligned;"
-                 : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]),
-                   "+f"(v[8]), "+f"(v[9]), "+f"(v[10]), "+f"(v[11]), "+f"(v[12]), "+f"(v[13]), "+f"(v[14]), "+f"(v[15]));
-}
-
 // Programmatic dependent launch: a kernel launched with the stream-serialisation attribute may start while
 // its predecessor in the stream is still running; it must not touch anything the predecessor (or any earlier
 // work) writes before pdl_wait() returns.  Both are no-ops in a plain launch.
@@ -186,58 +173,5 @@ __host__ __device__ constexpr int brev(int j) {
     return r;
 }
 __host__ __device__ constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
-
-// cos(2 pi k / 32), k = 0..8, correctly rounded to fp32 from float64.
-template <int K> struct Cos32Tab;
-template <> struct Cos32Tab<0> { static constexpr float v = 1.0f; };
-template <> struct Cos32Tab<1> { static constexpr float v = 0.98078528040323044913f; };
-template <> struct Cos32Tab<2> { static constexpr float v = 0.92387953251128675613f; };
-template <> struct Cos32Tab<3> { static constexpr float v = 0.83146961230254523708f; };
-template <> struct Cos32Tab<4> { static constexpr float v = 0.70710678118654752440f; };
-template <> struct Cos32Tab<5> { static constexpr float v = 0.55557023301960222474f; };
-template <> struct Cos32Tab<6> { static constexpr float v = 0.38268343236508977173f; };
-template <> struct Cos32Tab<7> { static constexpr float v = 0.19509032201612826785f; };
-template <> struct Cos32Tab<8> { static constexpr float v = 0.0f; };
-
-template <int K>
-__host__ __device__ constexpr float cos32() {
-    constexpr int k = ((K % 32) + 32) % 32;
-    if constexpr (k > 16) return cos32<32 - k>();
-    else if constexpr (k > 8) return -Cos32Tab<16 - k>::v;
-    else return Cos32Tab<k>::v;
-}
-template <int K>
-__host__ __device__ constexpr float sin32() { return cos32<K + 24>(); }   // sin(x) = cos(x - pi/2)
-
-// d * W_32^K,  W_32 = exp(-2 pi i / 32),  0 <= K < 16
-template <int K>
-__device__ __forceinline__ float2 mul_w32(float2 d) {
-    if constexpr (K == 0) return d;
-    else if constexpr (K == 8) return make_float2(d.y, -d.x);                     // * (-i)
-    else if constexpr (K == 4) { constexpr float c = Cos32Tab<4>::v; return make_float2(c * (d.x + d.y), c * (d.y - d.x)); }
-    else if constexpr (K == 12) { constexpr float c = Cos32Tab<4>::v; return make_float2(c * (d.y - d.x), -c * (d.x + d.y)); }
-    else {
-        constexpr float c = cos32<K>(), s = sin32<K>();                           // W = c - i s
-        return make_float2(d.x * c + d.y * s, d.y * c - d.x * s);
-    }
-}
-
-// In-register radix-2 decimation-in-frequency DFT of R points (R = 2..32, power of two):
-// on return v[j] = X[brev(j)] with X[k] = sum_t v_in[t] exp(-2 pi i k t / R).
-template <int R>
-__device__ __forceinline__ void dft_dif(float2 (&v)[R]) {
-    constexpr int LOG = ilog2(R);
-    sfor<0, LOG>([&](auto s_) {
-        constexpr int half = R >> (decltype(s_)::value + 1);
-        sfor<0, R / 2>([&](auto b_) {
-            constexpr int b = decltype(b_)::value;
-            constexpr int k = b % half;
-            constexpr int i = (b / half) * 2 * half + k;
-            float2 a = v[i], c = v[i + half];
-            v[i] = cadd(a, c);
-            v[i + half] = mul_w32<k * (16 / half)>(csub(a, c));   // W_{2 half}^k
-        });
-    });
-}
 
 }  // namespace plspec

@@ -199,10 +199,6 @@ __device__ __forceinline__ void bfly_dif_halves(float2 &r, float2 &i) {
     }
 }
 
-__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
 // ------------------------------------------------------------------------------------------
 // ST = true: the samples of IPP p that the CTA's gates touch (one contiguous run, overlapping windows
 // included once) are copied global -> shared by one cp.async.bulk per 32 KB while the CTA is still
