@@ -198,6 +198,8 @@ def main():
                          "integration sharded by IPP (sum all-reduce of S) / by range gate (all-gather)")
     ap.add_argument("--split", type=int, default=1, help="N > 16384: 1 decode pre-pass + scratch, 0 fully fused")
     ap.add_argument("--stage", type=int, default=1, help="1 shared-memory voltage stage where gates share samples, 2 wherever it fits, 0 direct loads")
+    ap.add_argument("--shared-code", action="store_true",
+                    help="workloads whose code repeats every IPP (cfg4's chirp): pass the one code (PLSPEC_OPT_SHARED_CODE)")
     ap.add_argument("--n-ipp", type=int, default=0, help="experiments: override the workload's IPP count")
     ap.add_argument("--n-ranges", type=int, default=0, help="experiments: override the workload's gate count")
     args = ap.parse_args()
@@ -241,13 +243,16 @@ def main():
         gs = shard.gate_shard(w.n_ranges, w.r0, w.stride, w.code_len, rank, world)
         rows_local, r0_local = gs.n_ranges, gs.r0
     V_pin = torch.from_numpy(np.ascontiguousarray(V_np)).pin_memory()
-    C_pin = torch.from_numpy(np.ascontiguousarray(C_np)).pin_memory()
+    shared_code = bool(args.shared_code)
+    if shared_code and not (C_np == C_np[:1]).all():
+        raise SystemExit(f"--shared-code: the codes of {w.name} differ from IPP to IPP")
+    C_pin = torch.from_numpy(np.ascontiguousarray(C_np[0] if shared_code else C_np)).pin_memory()
     V_dev, C_dev = V_pin.cuda(), C_pin.cuda()
     S_dev = torch.empty((rows_local, w.N), dtype=torch.float32, device="cuda")
     S_pin = torch.empty((rows_local, w.N), dtype=torch.float32).pin_memory()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     it = pl.Integrator(w.N, w.code_len, rows_local, r0_local, w.stride, w.ipp_len, w.dtype, kernel=args.kernel,
-                       ipp_chunks=args.chunks, stage=args.stage, split=args.split)
+                       ipp_chunks=args.chunks, stage=args.stage, split=args.split, shared_code=int(shared_code))
 
     def exchange(S):
         if mode == "ipp":
@@ -319,7 +324,8 @@ def main():
     cufft = None
     if world == 1 and not args.no_cufft:
         try:
-            cms, S_cu = cufft_pipeline(w, V_dev, C_dev, max(1, min(args.steps, 3)), flush)
+            cms, S_cu = cufft_pipeline(w, V_dev, C_dev.expand(w.n_ipp, -1) if shared_code else C_dev,
+                                       max(1, min(args.steps, 3)), flush)
             step_device()
             ref = S_cu.mean(dim=1, keepdim=True)
             dev = float(((S_dev - S_cu).abs() / ref).max())
@@ -339,7 +345,7 @@ def main():
         windows_per_step = w.windows * (world if mode == "replicas" else 1)
         value = windows_per_step * args.steps / (total_ms * 1e-3)
         esz = 4 if w.dtype == synth.SC16 else 8
-        h2d = w.n_ipp * (w.span * esz + w.code_len * 8)
+        h2d = w.n_ipp * w.span * esz + (1 if shared_code else w.n_ipp) * w.code_len * 8
         flops_per_launch = w.fft_flops                              # 5 N log2 N x windows of one launch
         achieved = flops_per_launch / (kern_mean * 1e-3) / 1e12
         traffic = None
@@ -362,7 +368,7 @@ def main():
                        "parallelism": (f"{world} independent integrations (one per GPU)" if mode == "replicas" else
                                        f"one integration sharded by {mode} over {world} GPUs"),
                        "kernel": {1: "generic", 2: "fused"}[stats["kernel_kind"]],
-                       "ipp_chunks": stats["ipp_chunks_last"]},
+                       "ipp_chunks": stats["ipp_chunks_last"], "shared_code": shared_code},
             "realtime_factor": w.data_seconds * (world if mode == "replicas" else 1) * args.steps / (total_ms * 1e-3),
             "wall_s_timed_region": wall_s,
             "clocks": clocks,

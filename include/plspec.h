@@ -59,6 +59,10 @@ enum { PLSPEC_OPT_KERNEL     = 1,   /* [0] 0 = auto, 1 = generic radix-2 kernel,
                                        with bulk asynchronous copies whenever the run of samples one CTA needs
                                        fits (N <= 16384 and, for complex64 input, N <= 8192); 0 = it always
                                        loads voltages straight from global memory.  Results are identical.  */
+       PLSPEC_OPT_SHARED_CODE = 7, /* [0] 1 = `codes` of plspec_accumulate holds ONE code of code_len samples that
+                                       decodes every IPP of the call (a transmitter that repeats its waveform, e.g.
+                                       the chirp of BASELINE config 4); 0 = codes[n_ipp][code_len], one per IPP.
+                                                                                            */
        PLSPEC_OPT_SPLIT      = 6 }; /* [1] N > 16384 only.  1 = every window is decoded once by a pre-pass kernel (with
                                        the outer radix-N/16384 butterfly) into a device scratch buffer (<= 4 GiB,
                                        IPPs batched to fit) and the fused kernel transforms the N/16384 residues

@@ -36,7 +36,7 @@ struct plspec_ctx {
     int kind = 2;                    // 1 generic, 2 fused
     int Nk = 0, Q = 1, RA = 1;   // N = Q * Nk, Nk = 1024 * RA (fused)
     int gates_per_cta = 1, n_groups = 0;
-    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1, opt_stage = 1, opt_split = 1;
+    int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1, opt_stage = 1, opt_split = 1, opt_shared_code = 0;
     // split path for N > 16384 (fused kernel only): decode + outer butterfly once into `xq`, then the
     // Q == 1 fused kernel over R * Q virtual gates of length Nk
     bool split = false;
@@ -58,6 +58,8 @@ struct plspec_ctx {
     long long cbits_words = 0;
     int *not_bpsk = nullptr;         // device flag written by pack_codes_kernel
     int epoch = 0;                   // number of the last code pre-pass
+    float2 *crep = nullptr;          // shared-code mode: the call's one code, one row per IPP
+    long long crep_elems = 0;
     // host pipeline
     cudaStream_t copy_stream = nullptr;
     Slot slot[kSlots];
@@ -193,8 +195,31 @@ cudaError_t launch_fused(const void *func, unsigned grid, unsigned block, void *
     return cudaLaunchKernelExC(&cfg, func, args);
 }
 
+// PLSPEC_OPT_SHARED_CODE: the one code of the call is spread over n_ipp rows of a device buffer, so that every
+// kernel keeps its one-code-per-IPP indexing (what the mode saves is the caller's memory and the H2D copy).
+__global__ void replicate_code_kernel(const float2 *__restrict__ code, float2 *__restrict__ rows, int L, long long total) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x)
+        rows[i] = __ldg(code + (int)(i % L));
+}
+
 int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0,
                       int n_ipp, cudaStream_t stream) {
+    if (h->opt_shared_code) {
+        const long long total = (long long)n_ipp * h->L;
+        if (total > h->crep_elems) {
+            if (h->crep) cudaFree(h->crep);
+            h->crep = nullptr; h->crep_elems = 0;
+            if (cudaMalloc((void **)&h->crep, sizeof(float2) * (size_t)total) != cudaSuccess) {
+                (void)cudaGetLastError();
+                return PLSPEC_ERR_ALLOC;
+            }
+            h->crep_elems = total;
+        }
+        replicate_code_kernel<<<h->n_sm * 4, 256, 0, stream>>>(dC, h->crep, h->L, total);
+        PL_CUDA(h, cudaGetLastError());
+        h->stats.kernel_launches++;
+        dC = h->crep;
+    }
     if (h->kind == 2 && h->split) return launch_split(h, dV, dC, v_pitch, r0, n_ipp, stream);
     KParams P;
     P.V = dV; P.C = dC; P.S = h->S; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
@@ -363,7 +388,7 @@ int ensure_slots(plspec_ctx *h, int batch) {
 // on the copy stream, overlapped with the kernels of earlier batches (PAPER.md:149 item 2).
 int accumulate_from_host(plspec_ctx *h, const void *V, const void *C, int n_ipp, cudaStream_t stream) {
     const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
-    const size_t per_ipp = (size_t)h->span * esz + (size_t)h->L * sizeof(float2);
+    const size_t per_ipp = (size_t)h->span * esz + (h->opt_shared_code ? 0 : (size_t)h->L * sizeof(float2));
     // auto: eight batches per call, but none below ~4 MB (each batch pays the launches' fixed cost once)
     int batch = (n_ipp + 7) / 8;
     const int min_batch = (int)(((size_t)4 << 20) / per_ipp) + 1;
@@ -383,9 +408,10 @@ int accumulate_from_host(plspec_ctx *h, const void *V, const void *C, int n_ipp,
         const char *src = (const char *)V + ((size_t)p0 * h->ipp_len + h->r0) * esz;
         PL_CUDA(h, cudaMemcpy2DAsync(sl.V, (size_t)h->span * esz, src, (size_t)h->ipp_len * esz,
                                      (size_t)h->span * esz, nb, cudaMemcpyHostToDevice, h->copy_stream));
-        PL_CUDA(h, cudaMemcpyAsync(sl.C, (const char *)C + (size_t)p0 * h->L * sizeof(float2),
-                                   (size_t)nb * h->L * sizeof(float2), cudaMemcpyHostToDevice, h->copy_stream));
-        h->stats.h2d_bytes += (long long)nb * (long long)per_ipp;
+        const size_t c_off = h->opt_shared_code ? 0 : (size_t)p0 * h->L * sizeof(float2);
+        const size_t c_bytes = (size_t)(h->opt_shared_code ? 1 : nb) * h->L * sizeof(float2);
+        PL_CUDA(h, cudaMemcpyAsync(sl.C, (const char *)C + c_off, c_bytes, cudaMemcpyHostToDevice, h->copy_stream));
+        h->stats.h2d_bytes += (long long)nb * (long long)h->span * (long long)esz + (long long)c_bytes;
         PL_CUDA(h, cudaEventRecord(sl.ready, h->copy_stream));
         PL_CUDA(h, cudaStreamWaitEvent(stream, sl.ready, 0));
         rc = launch_accumulate(h, sl.V, sl.C, h->span, 0, nb, stream);
@@ -456,6 +482,7 @@ void free_ctx(plspec_ctx *h) {
     if (h->twN) cudaFree(h->twN);
     if (h->cbits) cudaFree(h->cbits);
     if (h->xq) cudaFree(h->xq);
+    if (h->crep) cudaFree(h->crep);
     if (h->zero_bits) cudaFree(h->zero_bits);
     if (h->not_bpsk) cudaFree(h->not_bpsk);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
@@ -536,6 +563,10 @@ int plspec_configure(plspec_handle h, int option, int value) {
         case PLSPEC_OPT_IPP_CHUNKS: h->opt_chunks = value; return PLSPEC_OK;
         case PLSPEC_OPT_H2D_BATCH:  h->opt_batch = value;  return PLSPEC_OK;
         case PLSPEC_OPT_BPSK_PACK:  if (value > 1) return PLSPEC_ERR_INVALID_ARG; h->opt_bpsk = value; return PLSPEC_OK;
+        case PLSPEC_OPT_SHARED_CODE:
+            if (value > 1) return PLSPEC_ERR_INVALID_ARG;
+            h->opt_shared_code = value;
+            return PLSPEC_OK;
         case PLSPEC_OPT_SPLIT: {
             if (value > 1) return PLSPEC_ERR_INVALID_ARG;
             if (h->have_work) return PLSPEC_ERR_INVALID_ARG;

@@ -332,3 +332,28 @@ def test_repeated_runs_agree(N, dtype):
             first = S_gpu
         else:
             assert np.abs(S_gpu - first).max() <= 1e-6 * S_ref.mean()
+
+
+@pytest.mark.parametrize("N,dtype,complex_code,kernel", [
+    (256, synth.CF32, True, pl.KERNEL_GENERIC), (4096, synth.CF32, False, pl.KERNEL_AUTO),
+    (8192, synth.SC16, True, pl.KERNEL_AUTO), (16384, synth.SC16, False, pl.KERNEL_AUTO),
+    (16384, synth.CF32, True, pl.KERNEL_AUTO), (65536, synth.CF32, True, pl.KERNEL_AUTO)])
+@pytest.mark.parametrize("where", ["device", "pinned"])
+def test_shared_code_mode(N, dtype, complex_code, kernel, where):
+    """PLSPEC_OPT_SHARED_CODE: one code for every IPP == that code repeated per IPP."""
+    w, V, C = random_case(N, N, 21, 1, 2, 5, dtype, complex_code=complex_code)
+    C[:] = C[0]                                      # the transmitter repeats its waveform
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    S = torch.full((w.n_ranges, w.N), -1.0, dtype=torch.float32, device="cuda")
+    with pl.Integrator.for_workload(w, kernel=kernel, shared_code=1) as it:
+        keep = []                                    # host buffers stay valid until finalize
+        for a, b in ((0, 2), (2, 5)):                # two calls, the same single code each time
+            if where == "device":
+                v, c = to_dev(V[a:b]), to_dev(C[0])
+            else:
+                v = torch.from_numpy(np.ascontiguousarray(V[a:b])).pin_memory()
+                c = torch.from_numpy(np.ascontiguousarray(C[0])).pin_memory()
+            keep.append((v, c))
+            it.accumulate(v, c, b - a)
+        it.finalize(S)
+    assert gate_metric(S.cpu().numpy(), S_ref).max() <= TOL
