@@ -60,3 +60,17 @@ def test_binding_has_no_compute():
     src = open(os.path.join(ROOT, "paper_2311_18737_b200", "binding.py")).read()
     for banned in ("np.fft", "torch.fft", "np.abs", "np.conj", "oracle"):
         assert banned not in src.split('"""', 2)[2], banned
+
+
+def test_header_and_binding_constants_agree():
+    """Every PLSPEC_* enumerator of include/plspec.h has the same value in the binding."""
+    src = open(os.path.join(ROOT, "include", "plspec.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    consts = dict((k, int(v)) for k, v in re.findall(r"\b(PLSPEC_[A-Z0-9_]+)\s*=\s*(-?\d+)", src))
+    assert {"PLSPEC_OK", "PLSPEC_SC16", "PLSPEC_OPT_SPLIT", "PLSPEC_OPT_SHARED_CODE"} <= set(consts)
+    for name, value in consts.items():
+        if hasattr(pl, name):
+            assert getattr(pl, name) == value, name
+    for name in ("PLSPEC_OPT_KERNEL", "PLSPEC_OPT_IPP_CHUNKS", "PLSPEC_OPT_H2D_BATCH", "PLSPEC_OPT_BPSK_PACK",
+                 "PLSPEC_OPT_STAGE", "PLSPEC_OPT_SPLIT", "PLSPEC_OPT_SHARED_CODE"):
+        assert getattr(pl, name) == consts[name], name
