@@ -143,6 +143,21 @@ int plspec_finalize(plspec_handle h, float *S_out);
 int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, int guard,
                    int *k_up, float *p_up, int *k_dn, float *p_dn, float *noise, void *stream);
 
+/*
+ * EXTENSION ("mean P = S/P (Eq. 8), optional fftshift"): the mean power spectrum of a
+ * finished integration, PAPER.md:79 (Eq. 8: the estimate is the AVERAGE <|x|^2>; the hot path keeps the plain
+ * sum, reading A2), optionally with zero frequency moved to the middle of every row.
+ *   S         [device] S[n_ranges][N] as written by plspec_finalize, 16-byte aligned
+ *   P_out     [device] float[n_ranges][N], 16-byte aligned, must not alias S:
+ *             P_out[r][g] = S[r][f] / n_ipp (one IEEE float32 division), with g = f when centred = 0 and
+ *             g = (f + N/2) mod N when centred = 1 (DC at column N/2, negative frequencies to its left)
+ *   n_ipp     pulses summed in S (>= 1); 1 gives the plain (shifted) copy
+ *   stream    cudaStream_t; one kernel is enqueued and the call returns without synchronising
+ * Caller owns both buffers.  Errors: PLSPEC_ERR_INVALID_ARG (null, host, misaligned or aliased pointer, N not a
+ * power of two >= 16, n_ranges < 1, n_ipp < 1, centred not 0/1), PLSPEC_ERR_CUDA.  Needs no handle.
+ */
+int plspec_mean_spectrum(const float *S, float *P_out, int n_ranges, int N, int n_ipp, int centred, void *stream);
+
 /* EXTENSIONS ------------------------------------------------------------------------------- */
 int plspec_reset(plspec_handle h);                        /* zero the accumulators, no output */
 int plspec_destroy(plspec_handle h);                      /* free everything; NULL is OK       */

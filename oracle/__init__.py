@@ -6,7 +6,7 @@ It shares nothing with ``paper_2311_18737_b200`` (the CUDA path) and neither imp
 the other.  See ``oracle/plspec_oracle.c`` for the arithmetic and its citations
 (Eq. 8).
 """
-from .profile_oracle import profile  # noqa: F401
+from .profile_oracle import mean_spectrum, profile  # noqa: F401
 from .plspec_oracle import (  # noqa: F401
     CF32,
     SC16,

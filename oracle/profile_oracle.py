@@ -46,3 +46,20 @@ def profile(S, n_ipp: int, k_min: int, guard: int):
             cnt += 1
         noise[r] = np.float32(acc / cnt / n_ipp) if cnt else np.float32(0)
     return k_up, p_up, k_dn, p_dn, noise
+
+
+def mean_spectrum(S, n_ipp: int, centred: bool = False):
+    """Mean power spectrum, Eq. 8: P[r][f] = S[r][f] / n_ipp, written out bin by bin; with
+    ``centred`` bin f goes to column (f + N/2) mod N, so that DC sits at column N/2 and the negative
+    frequencies (bins above N/2, reading A9) to its left -- the usual centred display of a spectrum.  float32
+    division, as the GPU does it: the inputs are float32."""
+    S = np.asarray(S)
+    if S.dtype != np.float32 or S.ndim != 2 or n_ipp < 1:
+        raise ValueError("S must be float32 [n_ranges][N], n_ipp >= 1")
+    R, N = S.shape
+    P = np.zeros((R, N), np.float32)
+    for r in range(R):
+        for f in range(N):
+            g = (f + N // 2) % N if centred else f
+            P[r, g] = S[r, f] / np.float32(n_ipp)
+    return P

@@ -38,7 +38,8 @@ LIB_PATH = os.path.join(_HERE, "libplspec.so")
 # every symbol include/plspec.h declares (tests check the library exports each one)
 EXPORTED_SYMBOLS = (
     "plspec_create", "plspec_accumulate", "plspec_finalize", "plspec_reset", "plspec_destroy",
-    "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_profile", "plspec_strerror",
+    "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_profile", "plspec_mean_spectrum",
+    "plspec_strerror",
     "plspec_version",
 )
 
@@ -88,6 +89,7 @@ def lib() -> ctypes.CDLL:
         L.plspec_strerror.restype = ctypes.c_char_p
         L.plspec_version.restype = ctypes.c_char_p
         L.plspec_profile.argtypes = [vp, ci, ci, ci, ci, ci, vp, vp, vp, vp, vp, vp]
+        L.plspec_mean_spectrum.argtypes = [vp, vp, ci, ci, ci, ci, vp]
         for name in EXPORTED_SYMBOLS[:9]:
             getattr(L, name).restype = ci
         _lib = L
@@ -153,6 +155,11 @@ def plspec_profile(S, n_ranges, N, n_ipp, k_min, guard, k_up, p_up, k_dn, p_dn, 
     _check(None, lib().plspec_profile(_ptr(S), int(n_ranges), int(N), int(n_ipp), int(k_min), int(guard), _ptr(k_up),
                                       _ptr(p_up), _ptr(k_dn), _ptr(p_dn), _ptr(noise), _stream_ptr(stream)),
            "plspec_profile")
+
+
+def plspec_mean_spectrum(S, P_out, n_ranges, N, n_ipp, centred=False, stream=None) -> None:
+    _check(None, lib().plspec_mean_spectrum(_ptr(S), _ptr(P_out), int(n_ranges), int(N), int(n_ipp), int(bool(centred)),
+                                            _stream_ptr(stream)), "plspec_mean_spectrum")
 
 
 def plspec_reset(h) -> None:

@@ -657,6 +657,26 @@ int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, in
     return PLSPEC_OK;
 }
 
+int plspec_mean_spectrum(const float *S, float *P_out, int n_ranges, int N, int n_ipp, int centred, void *stream) {
+    if (!S || !P_out || S == P_out) return PLSPEC_ERR_INVALID_ARG;
+    if (!is_pow2(N) || N < 16 || n_ranges < 1 || n_ipp < 1 || (centred != 0 && centred != 1))
+        return PLSPEC_ERR_INVALID_ARG;
+    const void *ptrs[] = {S, P_out};
+    for (const void *p : ptrs) {                         // device (or managed) memory only, 16-byte aligned
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { (void)cudaGetLastError(); return PLSPEC_ERR_CUDA; }
+        if (a.type != cudaMemoryTypeDevice && a.type != cudaMemoryTypeManaged) return PLSPEC_ERR_INVALID_ARG;
+        if ((uintptr_t)p & 15) return PLSPEC_ERR_INVALID_ARG;
+    }
+    const long long n_vec = (long long)n_ranges * (N / 4);
+    long long blocks = (n_vec + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;              // grid-stride: eight CTAs of 256 per SM
+    mean_spectrum_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>((const float4 *)S, (float4 *)P_out, n_vec,
+                                                                             ilog2(N), n_ipp, centred);
+    if (cudaGetLastError() != cudaSuccess) return PLSPEC_ERR_CUDA;
+    return PLSPEC_OK;
+}
+
 int plspec_reset(plspec_handle h) {
     if (!h) return PLSPEC_ERR_INVALID_ARG;
     cudaStream_t st = h->last_stream;

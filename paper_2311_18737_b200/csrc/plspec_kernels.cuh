@@ -243,6 +243,24 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
     }
 }
 
+// Mean spectrum (Eq. 8, the AVERAGE power), optionally with the zero
+// frequency moved to the centre of each row: P[r][g] = S[r][f] / n_ipp, g = f (natural order) or
+// g = (f + N/2) mod N (centred).  One read and one write of R N floats, 128-bit and contiguous on both sides
+// (N/2 is a multiple of 4): HBM-bound, 8 B per bin.  IEEE division, so that x / 1 = x and both sides of the
+// parity test round alike.
+__global__ void __launch_bounds__(256) mean_spectrum_kernel(const float4 *__restrict__ S, float4 *__restrict__ P,
+                                                            long long n_vec, int log2N, int n_ipp, int centred) {
+    const float d = (float)n_ipp;
+    const int nv_row = 1 << (log2N - 2), half = centred ? nv_row >> 1 : 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_vec; i += (long long)gridDim.x * blockDim.x) {
+        float4 v = __ldcs(S + i);
+        v.x = __fdiv_rn(v.x, d); v.y = __fdiv_rn(v.y, d); v.z = __fdiv_rn(v.z, d); v.w = __fdiv_rn(v.w, d);
+        const long long row = i >> (log2N - 2);
+        const int c = (int)(i & (nv_row - 1));
+        __stcs(P + (row << (log2N - 2)) + ((c + half) & (nv_row - 1)), v);
+    }
+}
+
 __device__ __forceinline__ void tile_of_block(const KParams &P, int &r, int &q, int &p_begin, int &p_end) {
     int tile = blockIdx.x;
     r = tile % P.R;

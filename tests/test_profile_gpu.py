@@ -90,3 +90,51 @@ def test_user_stream_and_argument_errors():
         pl.plspec_profile(np.ones((3, 64), np.float32), 3, 64, 1, 2, 0, ki, pf, ki, pf, pf)
     with pytest.raises(pl.PlspecError):
         pl.plspec_profile(Sd, 3, 64, 1, 2, 0, None, pf, ki, pf, pf)
+
+
+@pytest.mark.parametrize("N,R", [(16, 1), (64, 37), (1024, 13), (4096, 301), (65536, 7)])
+@pytest.mark.parametrize("centred", [False, True])
+def test_mean_spectrum_parity(N, R, centred):
+    """plspec_mean_spectrum against oracle.mean_spectrum: bit-exact (one IEEE float32 division per bin on both
+    sides, the rest is addressing).  Shapes span one vector per thread to several grid-stride rounds."""
+    rng = np.random.default_rng(N + R)
+    S = (rng.random((R, N), dtype=np.float32) * np.float32(1e6)).astype(np.float32)
+    Sd = torch.from_numpy(S).cuda()
+    for n_ipp in (1, 7, 1000):
+        Pd = torch.full_like(Sd, -1.0)
+        pl.plspec_mean_spectrum(Sd, Pd, R, N, n_ipp, centred)
+        torch.cuda.synchronize()
+        assert np.array_equal(Pd.cpu().numpy(), oracle.mean_spectrum(S, n_ipp, centred)), (n_ipp,)
+        assert np.array_equal(Sd.cpu().numpy(), S)                      # the input is left alone
+
+
+def test_mean_spectrum_of_an_integration():
+    """End to end on cfg 1: accumulate -> finalize -> centred mean; the injected tone (bin 100, gate 20) shows at
+    column 100 + N/2 and the values equal the oracle's product of the same finalized spectrum."""
+    w = synth.CONFIGS["cfg1"]
+    V, C = synth.make_inputs(w)
+    S = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+    with pl.Integrator.for_workload(w) as it:
+        it.accumulate(torch.from_numpy(V).cuda(), torch.from_numpy(C).cuda(), w.n_ipp)
+        it.finalize(S)
+    P = torch.empty_like(S)
+    pl.plspec_mean_spectrum(S, P, w.n_ranges, w.N, w.n_ipp, True)
+    torch.cuda.synchronize()
+    Ph = P.cpu().numpy()
+    assert np.array_equal(Ph, oracle.mean_spectrum(S.cpu().numpy(), w.n_ipp, True))
+    assert int(np.argmax(Ph[20])) == 100 + w.N // 2
+
+
+def test_mean_spectrum_argument_errors():
+    Sd = torch.ones((3, 64), dtype=torch.float32, device="cuda"); Pd = torch.empty_like(Sd)
+    bad = [dict(N=48), dict(N=8), dict(n_ranges=0), dict(n_ipp=0)]
+    for b in bad:
+        a = dict(n_ranges=3, N=64, n_ipp=1); a.update(b)
+        with pytest.raises(pl.PlspecError):
+            pl.plspec_mean_spectrum(Sd, Pd, a["n_ranges"], a["N"], a["n_ipp"], False)
+    with pytest.raises(pl.PlspecError):
+        pl.plspec_mean_spectrum(Sd, Sd, 3, 64, 1, True)                 # aliased
+    with pytest.raises(pl.PlspecError):
+        pl.plspec_mean_spectrum(np.ones((3, 64), np.float32), Pd, 3, 64, 1, False)   # host pointer
+    with pytest.raises(pl.PlspecError):
+        pl.plspec_mean_spectrum(Sd.view(-1)[1:65], Pd, 1, 64, 1, False)  # misaligned

@@ -73,3 +73,29 @@ def test_recovers_the_chapman_profile_of_the_generator():
     # windows overlapping almost fully) decoded to noise: L (1 + 23 snr), amplitudes redrawn per IPP
     expect = w.code_len * (1.0 + (w.n_ranges - 1) * w.snr)
     assert np.all(nz > 0.6 * expect) and np.all(nz < 1.5 * expect)
+
+
+def test_mean_spectrum_pins():
+    """oracle.mean_spectrum against things other than itself: numpy's fftshift (library special case, n_ipp = 1),
+    a hand-placed spectrum (where DC, Nyquist and bins +-1 must land), exact halving, and the centred frequency
+    axis: column g holds frequency g - N/2 in cycles per N samples."""
+    rng = np.random.default_rng(5)
+    S = rng.random((4, 64), dtype=np.float32)
+    assert np.array_equal(oracle.mean_spectrum(S, 1, centred=True), np.fft.fftshift(S, axes=1))
+    assert np.array_equal(oracle.mean_spectrum(S, 1, centred=False), S)
+    assert np.array_equal(oracle.mean_spectrum(S, 2, centred=False), S * np.float32(0.5))
+    N = 16
+    T = np.zeros((1, N), np.float32)
+    T[0, 0] = 8.0; T[0, 1] = 16.0; T[0, N - 1] = 24.0; T[0, N // 2] = 32.0
+    P = oracle.mean_spectrum(T, 8, centred=True)[0]
+    want = np.zeros(N, np.float32)
+    want[N // 2] = 1.0; want[N // 2 + 1] = 2.0; want[N // 2 - 1] = 3.0; want[0] = 4.0    # Nyquist = most negative
+    assert np.array_equal(P, want)
+    # a tone at signed frequency k shows at column k + N/2 of the centred periodogram
+    N = 128
+    for k in (-40, -1, 0, 7, 63):
+        x = np.exp(2j * np.pi * k * np.arange(N) / N)
+        per = (np.abs(np.fft.fft(x)) ** 2).astype(np.float32)[None, :]
+        assert int(np.argmax(oracle.mean_spectrum(per, 1, centred=True)[0])) == k + N // 2
+    with pytest.raises(ValueError):
+        oracle.mean_spectrum(S, 0)
