@@ -201,6 +201,37 @@ def cufft_pipeline(w, V_dev, C_dev, steps, flush):
     return float(np.mean(ms)), S
 
 
+def products_timing(w, S_dev, flush, reps=7):
+    """plspec_mean_spectrum (centred) and plspec_profile on the finished S: median of `reps` launches, L2 flushed
+    before each, CUDA events on the current stream.  Both are one pass over S: algorithmic bytes 8 and 4 per bin,
+    against the measured HBM copy peak (MEASURED_PEAKS.json, else the profiling guide's 6 550 GB/s fallback)."""
+    import torch
+    from paper_2311_18737_b200 import binding as pl
+    R, N = w.n_ranges, w.N
+    try:
+        peak, src = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json"
+    except Exception:
+        peak, src = 6550.0, "fallback (B200_PROFILING.md)"
+    P = torch.empty_like(S_dev)
+    ki = torch.empty((2, R), dtype=torch.int32, device="cuda"); pf = torch.empty((3, R), dtype=torch.float32, device="cuda")
+    calls = {"mean_spectrum_centred": (8, lambda: pl.plspec_mean_spectrum(S_dev, P, R, N, w.n_ipp, True)),
+             "profile": (4, lambda: pl.plspec_profile(S_dev, R, N, w.n_ipp, max(1, N // 256), 2, ki[0], pf[0], ki[1],
+                                                      pf[1], pf[2]))}
+    out = {"hbm_peak_gbs": peak, "peak_source": src}
+    for name, (bpb, call) in calls.items():
+        ts = []
+        for _ in range(reps + 2):
+            flush.fill_(3)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); call(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ms = float(np.median(ts[2:]))
+        gbs = bpb * R * N / ms / 1e6
+        out[name] = {"ms": ms, "bytes_per_bin": bpb, "GB/s": gbs, "frac": gbs / peak}
+    return out
+
+
 def run_reference(args, w):
     """--impl reference: the oracle (the only 'reference implementation' this tier has)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -379,6 +410,14 @@ def main():
         except Exception as e:                                      # comparison only: never fails the bench
             cufft = {"error": f"{type(e).__name__}: {e}"[:200]}
 
+    # ---- post-integration products on the finished spectrum (outside the timed region)
+    products = None
+    if world == 1:
+        try:
+            products = products_timing(w, S_dev, flush)
+        except Exception as e:                                      # reported beside the metric: never fails the bench
+            products = {"error": f"{type(e).__name__}: {e}"[:200]}
+
     # ---- max over ranks
     total_ms, e2e_max, kern_mean = shard.max_over_ranks([total_ms, e2e_ms or 0.0, float(np.mean(kern_ms))],
                                                         device="cuda")
@@ -432,6 +471,8 @@ def main():
                                               / (e2e_ms * 1e-3)}
         if cufft is not None:
             line["cufft_pipeline"] = cufft
+        if products is not None:
+            line["products"] = products
         if world == 1 and not args.no_cpu_baseline:
             cb, _ = cpu_oracle_sample(w, V_np, C_np)
             line["cpu_baseline"] = cb

@@ -127,7 +127,8 @@ int plspec_finalize(plspec_handle h, float *S_out);
  * EXTENSION (the step after the hot path): per range gate of a finished spectrum,
  * where the plasma lines are.  PAPER.md:40-45 (Eq. 1): the plasma line lies at +-f_r from the ion line, and
  * f_r follows the electron density with range; PAPER.md:79 (Eq. 8): the estimate is the AVERAGE power.
- *   S         [device] S[n_ranges][N] as written by plspec_finalize (sum over n_ipp pulses, natural bin order)
+ *   S         [device] S[n_ranges][N] as written by plspec_finalize (sum over n_ipp pulses, natural bin order),
+ *             16-byte aligned
  *   n_ipp     pulses summed in S (>= 1): reported powers are S / n_ipp
  *   k_min     1 <= k_min < N/2: bins |f| < k_min (DC and the ion line) are left out
  *   guard     >= 0: bins within `guard` of either line are left out of the noise floor
@@ -137,8 +138,8 @@ int plspec_finalize(plspec_handle h, float *S_out);
  *   p_up,p_dn [device] float[n_ranges]: S / n_ipp at those bins
  *   noise     [device] float[n_ranges]: mean of S / n_ipp over the other bins of [k_min, N - k_min] \ {N/2}
  *   stream    cudaStream_t; one kernel is enqueued and the call returns without synchronising
- * Caller owns every buffer.  Errors: PLSPEC_ERR_INVALID_ARG (null or host pointer, N not a power of two >= 16,
- * range errors), PLSPEC_ERR_CUDA.  Needs no handle.
+ * Caller owns every buffer.  Errors: PLSPEC_ERR_INVALID_ARG (null or host pointer, S misaligned, N not a power of two
+ * >= 16, range errors), PLSPEC_ERR_CUDA.  Needs no handle.
  */
 int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, int guard,
                    int *k_up, float *p_up, int *k_dn, float *p_dn, float *noise, void *stream);

@@ -195,51 +195,80 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
                                                       int *__restrict__ k_up, float *__restrict__ p_up,
                                                       int *__restrict__ k_dn, float *__restrict__ p_dn,
                                                       float *__restrict__ noise) {
+    // One pass over the row in 128-bit loads (four in flight per thread): both arg maxima and the float64 sum of
+    // every searched bin; the few bins within `guard` of the lines are then taken out of the sum again (they are
+    // still in L1/L2), so the row crosses HBM once.
     __shared__ ProfileBest sb[2][8];
     __shared__ double ssum[8];
     __shared__ int scnt[8];
     __shared__ int sk[2];
+    __shared__ double stotal;
     const float *row = S + (long long)blockIdx.x * N;
+    const float4 *row4 = reinterpret_cast<const float4 *>(row);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lo = k_min, hi = N - k_min, mid = N / 2, nv = N / 4;
     ProfileBest up = {-1.f, 0x7fffffff}, dn = {-1.f, 0x7fffffff};      // S >= 0: any bin beats the start value
-    for (int f = k_min + tid; f <= N - k_min; f += 256) {
-        const ProfileBest c = {row[f], f};
-        if (f < N / 2) up = better(up, c);
-        else if (f > N / 2) dn = better(dn, c);
+    double acc = 0.0;
+    auto take = [&](float v, int f) {
+        if (f >= lo && f <= hi && f != mid) {
+            const ProfileBest c = {v, f};
+            if (f < mid) up = better(up, c); else dn = better(dn, c);
+            acc += (double)v;
+        }
+    };
+    for (int i0 = tid; i0 < nv; i0 += 4 * 256) {
+        float4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            const int i = i0 + u * 256;
+            v[u] = i < nv ? __ldg(row4 + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            const int i = i0 + u * 256;
+            if (i < nv) { take(v[u].x, 4 * i); take(v[u].y, 4 * i + 1); take(v[u].z, 4 * i + 2); take(v[u].w, 4 * i + 3); }
+        }
     }
 #pragma unroll
     for (int o = 16; o; o >>= 1) {
         ProfileBest u = {__shfl_xor_sync(0xffffffffu, up.v, o), __shfl_xor_sync(0xffffffffu, up.k, o)};
         ProfileBest d = {__shfl_xor_sync(0xffffffffu, dn.v, o), __shfl_xor_sync(0xffffffffu, dn.k, o)};
         up = better(up, u); dn = better(dn, d);
+        acc += __shfl_xor_sync(0xffffffffu, acc, o);
     }
-    if (lane == 0) { sb[0][warp] = up; sb[1][warp] = dn; }
+    if (lane == 0) { sb[0][warp] = up; sb[1][warp] = dn; ssum[warp] = acc; }
     __syncthreads();
     if (tid == 0) {
-        for (int w = 1; w < 8; w++) { up = better(up, sb[0][w]); dn = better(dn, sb[1][w]); }
+        for (int w = 1; w < 8; w++) { up = better(up, sb[0][w]); dn = better(dn, sb[1][w]); acc += ssum[w]; }
         sk[0] = up.k; sk[1] = dn.k;
+        stotal = acc;
         k_up[blockIdx.x] = up.k; k_dn[blockIdx.x] = dn.k;
         p_up[blockIdx.x] = up.v / (float)n_ipp;
         p_dn[blockIdx.x] = dn.v / (float)n_ipp;
     }
     __syncthreads();
+    // the bins within `guard` of either line (each once, inside the searched range): at most 2 (2 guard + 1)
     const int ku = sk[0], kd = sk[1];
-    double acc = 0.0;
-    int cnt = 0;
-    for (int f = k_min + tid; f <= N - k_min; f += 256) {
-        const int du = f > ku ? f - ku : ku - f, dd = f > kd ? f - kd : kd - f;
-        if (f != N / 2 && du > guard && dd > guard) { acc += (double)row[f]; cnt++; }
+    const int g = guard < N ? guard : N, wlen = 2 * g + 1;
+    double ex = 0.0;
+    int nex = 0;
+    for (int j = tid; j < 2 * wlen; j += 256) {
+        const bool second = j >= wlen;
+        const int f = (second ? kd : ku) - g + (second ? j - wlen : j);
+        const int du = f > ku ? f - ku : ku - f;
+        if (f >= lo && f <= hi && f != mid && !(second && du <= g)) { ex += (double)row[f]; nex++; }
     }
 #pragma unroll
     for (int o = 16; o; o >>= 1) {
-        acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+        ex += __shfl_xor_sync(0xffffffffu, ex, o);
+        nex += __shfl_xor_sync(0xffffffffu, nex, o);
     }
-    if (lane == 0) { ssum[warp] = acc; scnt[warp] = cnt; }
+    if (lane == 0) { ssum[warp] = ex; scnt[warp] = nex; }
     __syncthreads();
     if (tid == 0) {
-        for (int w = 1; w < 8; w++) { acc += ssum[w]; cnt += scnt[w]; }
-        noise[blockIdx.x] = cnt ? (float)(acc / (double)cnt / (double)n_ipp) : 0.f;
+        for (int w = 1; w < 8; w++) { ex += ssum[w]; nex += scnt[w]; }
+        const int cnt = (hi - lo) - nex;                               // hi - lo + 1 searched bins less N/2
+        noise[blockIdx.x] = cnt > 0 ? (float)((stotal - ex) / (double)cnt / (double)n_ipp) : 0.f;
     }
 }
 
