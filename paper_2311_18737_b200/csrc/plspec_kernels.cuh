@@ -226,7 +226,18 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
 #pragma unroll
         for (int u = 0; u < 4; u++) {
             const int i = i0 + u * 256;
-            if (i < nv) { take(v[u].x, 4 * i); take(v[u].y, 4 * i + 1); take(v[u].z, 4 * i + 2); take(v[u].w, 4 * i + 3); }
+            if (i >= nv) continue;
+            const int f0 = 4 * i;
+            if (f0 >= lo && f0 + 3 <= hi && (f0 + 3 < mid || f0 > mid)) {   // interior vector: one candidate, one add
+                ProfileBest c = {v[u].x, f0};                            // strict >: the lowest bin wins a tie
+                if (v[u].y > c.v) c = {v[u].y, f0 + 1};
+                if (v[u].z > c.v) c = {v[u].z, f0 + 2};
+                if (v[u].w > c.v) c = {v[u].w, f0 + 3};
+                if (f0 < mid) up = better(up, c); else dn = better(dn, c);
+                acc += ((double)v[u].x + (double)v[u].y) + ((double)v[u].z + (double)v[u].w);
+            } else {
+                take(v[u].x, f0); take(v[u].y, f0 + 1); take(v[u].z, f0 + 2); take(v[u].w, f0 + 3);
+            }
         }
     }
 #pragma unroll
