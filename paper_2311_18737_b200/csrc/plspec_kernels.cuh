@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
                                                       int *__restrict__ k_up, float *__restrict__ p_up,
                                                       int *__restrict__ k_dn, float *__restrict__ p_dn,
                                                       float *__restrict__ noise) {
-    // One pass over the row in 128-bit loads (four in flight per thread): both arg maxima and the float64 sum of
+    // One pass over the row in 128-bit loads (eight in flight per thread): both arg maxima and the float64 sum of
     // every searched bin; the few bins within `guard` of the lines are then taken out of the sum again (they are
     // still in L1/L2), so the row crosses HBM once.
     __shared__ ProfileBest sb[2][8];
@@ -216,15 +216,15 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
             acc += (double)v;
         }
     };
-    for (int i0 = tid; i0 < nv; i0 += 4 * 256) {
-        float4 v[4];
+    for (int i0 = tid; i0 < nv; i0 += 8 * 256) {
+        float4 v[8];
 #pragma unroll
-        for (int u = 0; u < 4; u++) {
+        for (int u = 0; u < 8; u++) {
             const int i = i0 + u * 256;
             v[u] = i < nv ? __ldg(row4 + i) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
-        for (int u = 0; u < 4; u++) {
+        for (int u = 0; u < 8; u++) {
             const int i = i0 + u * 256;
             if (i >= nv) continue;
             const int f0 = 4 * i;
