@@ -138,3 +138,25 @@ def test_mean_spectrum_argument_errors():
         pl.plspec_mean_spectrum(np.ones((3, 64), np.float32), Pd, 3, 64, 1, False)   # host pointer
     with pytest.raises(pl.PlspecError):
         pl.plspec_mean_spectrum(Sd.view(-1)[1:65], Pd, 1, 64, 1, False)  # misaligned
+
+
+def test_products_on_a_user_stream_and_misaligned_profile_input():
+    """Both product calls enqueue on the caller's stream without synchronising; plspec_profile refuses a spectrum
+    that is not 16-byte aligned (its rows are read in 128-bit loads)."""
+    rng = np.random.default_rng(77)
+    S = rng.random((9, 256), dtype=np.float32)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        Sd = torch.from_numpy(S).cuda()
+        Pd = torch.empty_like(Sd)
+    st.synchronize()
+    pl.plspec_mean_spectrum(Sd, Pd, 9, 256, 3, True, st)
+    got = run(S, 3, 4, 1, stream=st)
+    st.synchronize()
+    assert np.array_equal(Pd.cpu().numpy(), oracle.mean_spectrum(S, 3, True))
+    ref = oracle.profile(S, 3, 4, 1)
+    assert np.array_equal(got[0], ref[0]) and np.array_equal(got[2], ref[2])
+    buf = torch.ones(64 * 3 + 4, dtype=torch.float32, device="cuda")
+    ki = torch.zeros(3, dtype=torch.int32, device="cuda"); pf = torch.zeros(3, dtype=torch.float32, device="cuda")
+    with pytest.raises(pl.PlspecError):
+        pl.plspec_profile(buf[1:], 3, 64, 1, 2, 0, ki, pf, ki, pf, pf)
