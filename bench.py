@@ -35,8 +35,9 @@ from paper_2311_18737_b200 import synth  # noqa: E402
 
 METRIC = "decoded range-gate spectra/s at N=16384"
 UNIT = "spectra/s"
-# FP32 ALU peak: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz max SM clock (B200_PROFILING.md
-# unit counts and clocks).  Measured FFMA issue rate on this pool: 124.6 of 128.
+# FP32 ALU peak, derived: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz max SM clock (B200_PROFILING.md
+# unit counts and clocks).  The MEASURED rate (plspec_diag_fp32_peak, run below under the
+# clock sampler) is printed beside it as roofline.peak_measured.
 N_SM, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
 ALU_PEAK_TFLOPS = N_SM * FP32_LANES * 2 * SM_MAX_GHZ / 1e3
 PAPER_BEST_SPECTRA_PER_S = 409600 / 1.488      # GTX 780 Ti, PAPER.md:139 (workload "paper" only)
@@ -165,40 +166,65 @@ def cpu_oracle_sample(w, V, C, target_s=12.0, steps=1):
 
 
 def cufft_pipeline(w, V_dev, C_dev, steps, flush):
-    """Comparison point, not the product (north_star): the unfused structure the paper describes
-     -- per IPP a decode multiply that writes `batch` to device memory, a batched cuFFT
-    (torch.fft -> cufftExecC2C) over its rows, and a power-accumulate pass -- on the same device-resident
-    inputs, timed with CUDA events like `value`."""
+    """Comparison point, not the product (north_star): the unfused structure the paper describes (PAPER.md:103-121)
+    as written -- per pulse a "complex multiplication" kernel that writes `batch[R][N]` to device memory, one
+    in-place batched cufftExecC2C over its rows (cufftPlanMany), and a "spectrum accumulation" kernel -- built
+    from csrc/cufft_pipeline.cu into libplspec_cufft.so, on the same device-resident inputs and timed with CUDA
+    events like `value` (spectrum zeroed inside the timed region, as finalize does for ours)."""
+    import ctypes
     import torch
-    R, L, N = w.n_ranges, w.code_len, w.N
-    S = torch.zeros((R, N), dtype=torch.float32, device="cuda")
+    from paper_2311_18737_b200 import build as plbuild
+    L = ctypes.CDLL(plbuild.build_cufft_pipeline())
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    L.plspec_cufft_create.argtypes = [ci, ci, ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
+    L.plspec_cufft_accumulate.argtypes = [vp, vp, vp, ci, vp, vp]
+    L.plspec_cufft_launches.argtypes = [vp]
+    L.plspec_cufft_launches.restype = ctypes.c_longlong
+    L.plspec_cufft_destroy.argtypes = [vp]
+    h = vp()
+    rc = L.plspec_cufft_create(w.N, w.code_len, w.n_ranges, w.r0, w.stride, w.ipp_len, w.dtype, ctypes.byref(h))
+    if rc != 0:
+        raise RuntimeError(f"plspec_cufft_create failed ({rc})")
+    S = torch.zeros((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
 
     def step():
         S.zero_()
-        for p in range(w.n_ipp):
-            if w.dtype == synth.SC16:
-                v = torch.view_as_complex(V_dev[p].to(torch.float32))          # sc16 -> fp32 (a1)
-            else:
-                v = V_dev[p]
-            win = v.as_strided((R, L), (w.stride, 1), v.storage_offset() + w.r0)   # overlapping windows (a2), a view
-            batch = win * C_dev[p].conj()                                       # K1 decode (a3)
-            X = torch.fft.fft(batch, n=N, dim=1)                                # K2 cuFFT, zero-padded to N (a4)
-            S.add_(torch.view_as_real(X).square().sum(dim=-1))                  # K3 power + accumulate (a5, a6)
-        return S
+        rc = L.plspec_cufft_accumulate(h, V_dev.data_ptr(), C_dev.data_ptr(), w.n_ipp, S.data_ptr(), stream)
+        if rc != 0:
+            raise RuntimeError(f"plspec_cufft_accumulate failed ({rc})")
 
-    for _ in range(2):
-        step()
-    torch.cuda.synchronize()
-    ms = []
-    for _ in range(steps):
-        flush.fill_(4)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        step()
-        e1.record()
-        e1.synchronize()
-        ms.append(e0.elapsed_time(e1))
+    try:
+        for _ in range(2):
+            step()
+        torch.cuda.synchronize()
+        ms = []
+        for _ in range(steps):
+            flush.fill_(4)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            step()
+            e1.record()
+            e1.synchronize()
+            ms.append(e0.elapsed_time(e1))
+    finally:
+        L.plspec_cufft_destroy(h)
     return float(np.mean(ms)), S
+
+
+def ncu_traffic(name):
+    """DRAM bytes per fused-kernel launch from the committed `ncu --set full` capture of this workload
+    (dram__bytes_read.sum + dram__bytes_write.sum), with the capture it came from; (None, why) if there is none.
+    The table sits beside the binding (paper_2311_18737_b200/ncu_traffic.json) and is refreshed by hand from
+    profiles/ whenever the kernels change: a number from a profiler run is evidence, never a bench value."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "paper_2311_18737_b200", "ncu_traffic.json")))
+        e = t["workloads"].get(name)
+        if e:
+            return int(e["dram_bytes_per_launch"]), e["source"]
+        return None, "no ncu capture of this workload committed"
+    except Exception as e:
+        return None, f"ncu_traffic.json unreadable: {type(e).__name__}"
 
 
 def products_timing(w, S_dev, flush, reps=7):
@@ -232,21 +258,34 @@ def products_timing(w, S_dev, flush, reps=7):
     return out
 
 
+def workload_config(w, l2, parallelism):
+    """The `config` object of the JSON line: what defines the workload, the same keys for both arms."""
+    return {"workload": w.name, "N": w.N, "code_len": w.code_len, "n_ranges": w.n_ranges, "stride": w.stride,
+            "n_ipp": w.n_ipp, "ipp_len": w.ipp_len, "input": "sc16" if w.dtype == synth.SC16 else "complex64",
+            "windows_per_step": w.windows, "l2": l2, "parallelism": parallelism}
+
+
 def run_reference(args, w):
-    """--impl reference: the oracle (the only 'reference implementation' this tier has)."""
+    """--impl reference: the oracle (the only 'reference implementation' this tier has), as it stands, on the
+    host cores.  Every one of the `warmup` + `steps` steps is run; each is a bounded sample of the workload (a
+    subset of gates over all IPPs) sized so that the whole run ends within about two minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     V, C = synth.make_inputs(w)
-    for _ in range(min(args.warmup, 1)):
-        cpu_oracle_sample(w, V, C, target_s=2.0)
-    cb, dt = cpu_oracle_sample(w, V, C, target_s=10.0, steps=max(1, min(args.steps, 5)))
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    per_step_s = min(10.0, 110.0 / (steps + warmup))
+    if warmup:
+        cpu_oracle_sample(w, V, C, target_s=per_step_s, steps=warmup)
+    cb, dt = cpu_oracle_sample(w, V, C, target_s=per_step_s, steps=steps)
     line = {
         "impl": "reference", "metric": metric_name(w), "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "steps": steps, "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "N": w.N, "n_ranges": w.n_ranges, "n_ipp": w.n_ipp,
-                   "note": "each step is a bounded sample of the workload (subset of gates, all IPPs)"},
+        "config": workload_config(w, "n/a (float64 oracle on the host cores)",
+                                  "oracle on rank 0's host cores (OpenMP over range gates)"),
+        "sample_note": "each step is a bounded sample of the workload (subset of gates, all IPPs); value = windows "
+                       "of the sample / its time",
         "cpu_baseline": cb,
         "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -264,7 +303,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT + elementwise comparison pipeline")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT comparison pipeline")
+    ap.add_argument("--no-peak", action="store_true", help="skip the FP32 peak micro-benchmark")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 fused")
     ap.add_argument("--chunks", type=int, default=0)
     ap.add_argument("--shard", default="replicas", choices=["replicas", "ipp", "gates"],
@@ -350,6 +390,19 @@ def main():
         if mode != "replicas":
             exchange(S_pin.cuda())
 
+    # ---- measured FP32 multiply-add peak (the roofline's measured denominator), clocks sampled meanwhile
+    peak_meas = None
+    if rank == 0 and not args.no_peak:
+        ps = ClockSampler(local)
+        ps.start()
+        pk2 = pl.plspec_diag_fp32_peak(packed=True, iters=1 << 16, reps=40)     # FFMA2: what the fused kernel issues
+        pk1 = pl.plspec_diag_fp32_peak(packed=False, iters=1 << 16, reps=40)    # scalar FFMA
+        pc = ps.stop()
+        peak_meas = {"ffma2_tflops_best": pk2["tflops_best"], "ffma2_tflops_mean": pk2["tflops_mean"],
+                     "ffma_tflops_best": pk1["tflops_best"], "ffma_tflops_mean": pk1["tflops_mean"], "clocks": pc,
+                     "how": "plspec_diag_fp32_peak: 4 x 512 threads per SM, 32 independent multiply-add chains per "
+                            "thread, 40 launches of 65536 iterations each, CUDA events"}
+
     # ---- device-resident timing
     for _ in range(args.warmup):
         flush.fill_(1)
@@ -398,14 +451,18 @@ def main():
     cufft = None
     if world == 1 and not args.no_cufft:
         try:
-            cms, S_cu = cufft_pipeline(w, V_dev, C_dev.expand(w.n_ipp, -1) if shared_code else C_dev,
+            cms, S_cu = cufft_pipeline(w, V_dev, C_dev.expand(w.n_ipp, -1).contiguous() if shared_code else C_dev,
                                        max(1, min(args.steps, 3)), flush)
             step_device()
             ref = S_cu.mean(dim=1, keepdim=True)
             dev = float(((S_dev - S_cu).abs() / ref).max())
+            decoded = w.windows * w.N
             cufft = {"ms_per_step": cms, "value": w.windows / (cms * 1e-3), "unit": UNIT,
                      "max_rel_dev_vs_fused": dev,
-                     "kind": "torch: decode multiply -> torch.fft.fft (cuFFT) -> power-accumulate, per IPP"}
+                     "model_dram_bytes_per_decoded_sample": 40, "model_ms_at_hbm_peak": decoded * 40 / 6.55e12 * 1e3,
+                     "kind": "csrc/cufft_pipeline.cu: complex_multiplication_kernel -> cufftPlanMany/cufftExecC2C "
+                             "in place over batch[R][N] -> spectrum_accumulation_kernel, looped per pulse "
+                             "(PAPER.md:105-121); device-resident inputs"}
             del S_cu
         except Exception as e:                                      # comparison only: never fails the bench
             cufft = {"error": f"{type(e).__name__}: {e}"[:200]}
@@ -428,41 +485,41 @@ def main():
         value = windows_per_step * args.steps / (total_ms * 1e-3)
         esz = 4 if w.dtype == synth.SC16 else 8
         h2d = w.n_ipp * w.span * esz + (1 if shared_code else w.n_ipp) * w.code_len * 8
-        flops_per_launch = w.fft_flops                              # 5 N log2 N x windows of one launch
+        # one launch of a sharded integration transforms this rank's share of the windows (kern_mean is the
+        # max over ranks of one rank's time); replicas each transform the whole workload
+        share = (n_ipp_local / w.n_ipp) * (rows_local / w.n_ranges)
+        flops_per_launch = w.fft_flops * share                      # 5 N log2 N x windows of one launch
         achieved = flops_per_launch / (kern_mean * 1e-3) / 1e12
-        traffic = None
-        tfile = os.path.join(ROOT, "profiles", "traffic_bytes.txt")
-        if os.path.exists(tfile):
-            try:
-                traffic = json.load(open(tfile)).get(w.name)
-            except Exception:
-                traffic = None
+        traffic, traffic_source = ncu_traffic(w.name) if share == 1.0 else (None, "sharded launch: not captured")
         line = {
             "metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak" if mode == "replicas" else "strong",
             "vs_baseline": (value / PAPER_BEST_SPECTRA_PER_S) if w.name == "paper" else None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "N": w.N, "code_len": w.code_len, "n_ranges": w.n_ranges,
-                       "stride": w.stride, "n_ipp": w.n_ipp, "ipp_len": w.ipp_len,
-                       "input": "sc16" if w.dtype == synth.SC16 else "complex64",
-                       "windows_per_step": w.windows, "l2": "flushed between steps (256 MB write)",
-                       "parallelism": (f"{world} independent integrations (one per GPU)" if mode == "replicas" else
-                                       f"one integration sharded by {mode} over {world} GPUs"),
-                       "kernel": {1: "generic", 2: "fused"}[stats["kernel_kind"]],
-                       "ipp_chunks": stats["ipp_chunks_last"], "shared_code": shared_code},
+            "config": workload_config(w, "flushed between steps (256 MB write)",
+                                      (f"{world} independent integrations (one per GPU)" if mode == "replicas" else
+                                       f"one integration sharded by {mode} over {world} GPUs")),
+            "impl_detail": {"kernel": {1: "generic", 2: "fused"}[stats["kernel_kind"]],
+                            "ipp_chunks": stats["ipp_chunks_last"], "shared_code": shared_code},
             "realtime_factor": w.data_seconds * (world if mode == "replicas" else 1) * args.steps / (total_ms * 1e-3),
             "wall_s_timed_region": wall_s,
             "clocks": clocks,
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
-                         "frac": achieved / ALU_PEAK_TFLOPS, "traffic": traffic,
+                         "frac": achieved / ALU_PEAK_TFLOPS, "traffic": traffic, "traffic_source": traffic_source,
                          "kernel": "fused_kernel" if stats["kernel_kind"] == 2 else "generic_kernel",
                          "kernel_ms": kern_mean, "flops_per_launch": flops_per_launch,
                          "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); "
                                         "MEASURED_PEAKS.json holds no FP32 ALU figure",
-                         "hbm_bytes_algorithmic": w.n_ipp * (w.ipp_len * esz + w.code_len * 8) + w.n_ranges * w.N * 4},
+                         "hbm_bytes_algorithmic": int((n_ipp_local * (w.ipp_len * esz + w.code_len * 8)
+                                                       + rows_local * w.N * 4))},
         }
+        if peak_meas is not None:
+            pm = peak_meas["ffma2_tflops_mean"]
+            line["roofline"].update({
+                "peak_measured": pm, "frac_of_measured": achieved / pm,
+                "peak_clock_mhz": peak_meas["clocks"].get("sm_mhz"), "peak_measurement": peak_meas})
         if e2e_ms is not None:
             line["e2e"] = {"value": windows_per_step * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
                            "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(w.n_ranges * w.N * 4),

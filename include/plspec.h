@@ -59,15 +59,16 @@ enum { PLSPEC_OPT_KERNEL     = 1,   /* [0] 0 = auto, 1 = generic radix-2 kernel,
                                        with bulk asynchronous copies whenever the run of samples one CTA needs
                                        fits (N <= 16384 and, for complex64 input, N <= 8192); 0 = it always
                                        loads voltages straight from global memory.  Results are identical.  */
-       PLSPEC_OPT_SHARED_CODE = 7, /* [0] 1 = `codes` of plspec_accumulate holds ONE code of code_len samples that
-                                       decodes every IPP of the call (a transmitter that repeats its waveform, e.g.
-                                       the chirp of BASELINE config 4); 0 = codes[n_ipp][code_len], one per IPP.
-                                       (SURVEY.md 8(f) NEXT-4)                                                     */
-       PLSPEC_OPT_SPLIT      = 6 }; /* [1] N > 16384 only.  1 = every window is decoded once by a pre-pass kernel (with
+       PLSPEC_OPT_SPLIT      = 6,   /* [1] N > 16384 only.  1 = every window is decoded once by a pre-pass kernel (with
                                        the outer radix-N/16384 butterfly) into a device scratch buffer (<= 4 GiB,
                                        IPPs batched to fit) and the fused kernel transforms the N/16384 residues
                                        as separate length-16384 windows; 0 = each (gate, residue) CTA decodes the
                                        whole window itself (no scratch, N/16384 times the loads).               */
+       PLSPEC_OPT_SHARED_CODE = 7   /* [0] 1 = `codes` of plspec_accumulate holds ONE code of code_len samples that
+                                       decodes every IPP of the call (a transmitter that repeats its waveform, e.g.
+                                       the chirp of BASELINE config 4); 0 = codes[n_ipp][code_len], one per IPP.
+                                       (SURVEY.md 8(f) NEXT-4)                                                     */
+     };
 
 /* Counters since create (EXTENSION; used by bench.py for gpu_launches / h2d bytes). */
 typedef struct {
@@ -139,7 +140,7 @@ int plspec_finalize(plspec_handle h, float *S_out);
  *   noise     [device] float[n_ranges]: mean of S / n_ipp over the other bins of [k_min, N - k_min] \ {N/2}
  *   stream    cudaStream_t; one kernel is enqueued and the call returns without synchronising
  * Caller owns every buffer.  Errors: PLSPEC_ERR_INVALID_ARG (null or host pointer, S misaligned, N not a power of two
- * >= 16, range errors), PLSPEC_ERR_CUDA.  Needs no handle.
+ * in [16, 65536], range errors), PLSPEC_ERR_CUDA.  Needs no handle.
  */
 int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, int guard,
                    int *k_up, float *p_up, int *k_dn, float *p_dn, float *noise, void *stream);
@@ -155,9 +156,24 @@ int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, in
  *   n_ipp     pulses summed in S (>= 1); 1 gives the plain (shifted) copy
  *   stream    cudaStream_t; one kernel is enqueued and the call returns without synchronising
  * Caller owns both buffers.  Errors: PLSPEC_ERR_INVALID_ARG (null, host, misaligned or aliased pointer, N not a
- * power of two >= 16, n_ranges < 1, n_ipp < 1, centred not 0/1), PLSPEC_ERR_CUDA.  Needs no handle.
+ * power of two in [16, 65536], n_ranges < 1, n_ipp < 1, centred not 0/1), PLSPEC_ERR_CUDA.  Needs no handle.
  */
 int plspec_mean_spectrum(const float *S, float *P_out, int n_ranges, int N, int n_ipp, int centred, void *stream);
+
+/*
+ * DIAGNOSTIC ("measured FMA peak to be reported beside" the derived one): the
+ * FP32 multiply-add issue rate of the current device, the measured denominator of the path's ALU roofline
+ * (5 N log2 N flop per decoded window).  Launches reps + 1 kernels of 4 x 512 threads per SM, each
+ * thread running 32 independent multiply-add chains for `iters` iterations (64 flop per thread and iteration; no
+ * memory traffic), times each with CUDA events on `stream` and blocks until done.
+ *   packed       0 = scalar FFMA, 1 = packed FFMA2 (two lanes per instruction: the form the fused kernel issues)
+ *   iters        >= 1 loop iterations per thread (1 << 16 gives launches of a few milliseconds)
+ *   reps         1 ... 100000 timed launches after one warm-up launch
+ *   tflops_best  [host] fastest launch, in TFLOP/s (2 flop per multiply-add)
+ *   tflops_mean  [host] mean over the `reps` launches (sustained rate when reps spans seconds)
+ * Errors: PLSPEC_ERR_INVALID_ARG, PLSPEC_ERR_ALLOC, PLSPEC_ERR_CUDA.  Needs no handle; touches no integrator state.
+ */
+int plspec_diag_fp32_peak(int packed, int iters, int reps, double *tflops_best, double *tflops_mean, void *stream);
 
 /* EXTENSIONS ------------------------------------------------------------------------------- */
 int plspec_reset(plspec_handle h);                        /* zero the accumulators, no output */

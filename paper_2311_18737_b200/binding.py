@@ -39,9 +39,11 @@ LIB_PATH = os.path.join(_HERE, "libplspec.so")
 EXPORTED_SYMBOLS = (
     "plspec_create", "plspec_accumulate", "plspec_finalize", "plspec_reset", "plspec_destroy",
     "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_profile", "plspec_mean_spectrum",
+    "plspec_diag_fp32_peak",
     "plspec_strerror",
     "plspec_version",
 )
+_INT_STATUS = EXPORTED_SYMBOLS[:-2]          # every call but strerror / version returns an int status
 
 
 class plspec_stats_t(ctypes.Structure):
@@ -90,7 +92,9 @@ def lib() -> ctypes.CDLL:
         L.plspec_version.restype = ctypes.c_char_p
         L.plspec_profile.argtypes = [vp, ci, ci, ci, ci, ci, vp, vp, vp, vp, vp, vp]
         L.plspec_mean_spectrum.argtypes = [vp, vp, ci, ci, ci, ci, vp]
-        for name in EXPORTED_SYMBOLS[:9]:
+        L.plspec_diag_fp32_peak.argtypes = [ci, ci, ci, ctypes.POINTER(ctypes.c_double),
+                                            ctypes.POINTER(ctypes.c_double), vp]
+        for name in _INT_STATUS:
             getattr(L, name).restype = ci
         _lib = L
     return _lib
@@ -160,6 +164,14 @@ def plspec_profile(S, n_ranges, N, n_ipp, k_min, guard, k_up, p_up, k_dn, p_dn, 
 def plspec_mean_spectrum(S, P_out, n_ranges, N, n_ipp, centred=False, stream=None) -> None:
     _check(None, lib().plspec_mean_spectrum(_ptr(S), _ptr(P_out), int(n_ranges), int(N), int(n_ipp), int(bool(centred)),
                                             _stream_ptr(stream)), "plspec_mean_spectrum")
+
+
+def plspec_diag_fp32_peak(packed=True, iters=1 << 16, reps=10, stream=None) -> dict:
+    """Measured FP32 multiply-add rate of the current device in TFLOP/s (best launch, mean over launches)."""
+    best, mean = ctypes.c_double(), ctypes.c_double()
+    _check(None, lib().plspec_diag_fp32_peak(int(bool(packed)), int(iters), int(reps), ctypes.byref(best),
+                                             ctypes.byref(mean), _stream_ptr(stream)), "plspec_diag_fp32_peak")
+    return {"tflops_best": best.value, "tflops_mean": mean.value}
 
 
 def plspec_reset(h) -> None:

@@ -56,7 +56,7 @@ struct plspec_ctx {
     float2 *twA = nullptr, *twB = nullptr, *twN = nullptr;
     uint32_t *cbits = nullptr;       // packed code signs of the launch in flight (BPSK fast path)
     long long cbits_words = 0;
-    int *not_bpsk = nullptr;         // device flag written by pack_codes_kernel
+    int *not_bpsk = nullptr;         // [0]: device flag written by pack_codes_kernel; [1]: never written, always 0
     int epoch = 0;                   // number of the last code pre-pass
     float2 *crep = nullptr;          // shared-code mode: the call's one code, one row per IPP
     long long crep_elems = 0;
@@ -87,6 +87,16 @@ namespace {
     } while (0)
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// SM count of the current device (the handle-free calls size their grids with it); 0 on error
+int device_sm_count() {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0;
+    }
+    return n;
+}
 
 template <int RA, int Q, bool ST>
 const void *fused_ptr(int dt) {
@@ -296,7 +306,6 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
             return PLSPEC_ERR_ALLOC;
         }
         PL_CUDA(h, cudaMemsetAsync(h->zero_bits, 0, sizeof(uint32_t) * (size_t)h->zero_bits_words, stream));
-        PL_CUDA(h, cudaMemsetAsync(h->not_bpsk, 0, sizeof(int), stream));
     }
     const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
     for (int p0 = 0; p0 < n_ipp; p0 += (int)h->xq_ipps) {
@@ -325,7 +334,9 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
         // step 2: R * Q virtual gates, window = Nk contiguous decoded samples, identity code
         KParams F = P;
         F.V = h->xq; F.C = dC;
-        F.Cbits = h->zero_bits; F.not_bpsk = h->not_bpsk;            // flag stays 0: sign-flip decode, no flips
+        // sign-flip decode, no flips.  The flag word is the handle's permanent zero, not the one pack_codes_kernel
+        // writes: an earlier launch of the unsplit path on this handle may have left any epoch in that one.
+        F.Cbits = h->zero_bits; F.not_bpsk = h->not_bpsk + 1; F.epoch = 1;
         F.v_pitch = per_ipp;
         F.N = h->Nk; F.Q = 1; F.L = h->Nk;
         F.R = h->R * h->Q; F.r0 = 0; F.stride = h->Nk;
@@ -528,7 +539,7 @@ int plspec_create(int N, int code_len, int n_ranges, int r0, int stride, int ipp
     cudaError_t e = cudaGetDevice(&h->device);
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, h->device);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete h; return PLSPEC_ERR_CUDA; }
-    if (prop.major < 10) { delete h; return PLSPEC_ERR_UNSUPPORTED; }   // sm_100a code only
+    if (prop.major != 10 || prop.minor != 0) { delete h; return PLSPEC_ERR_UNSUPPORTED; }   // the library holds sm_100a code only
     h->n_sm = prop.multiProcessorCount;
 
     auto fail = [&](int code) { free_ctx(h); return code; };
@@ -540,8 +551,8 @@ int plspec_create(int N, int code_len, int n_ranges, int r0, int stride, int ipp
         (void)cudaGetLastError();
         return fail(PLSPEC_ERR_CUDA);
     }
-    if (cudaMalloc((void **)&h->not_bpsk, sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_ALLOC); }
-    if (cudaMemset(h->not_bpsk, 0, sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_CUDA); }
+    if (cudaMalloc((void **)&h->not_bpsk, 2 * sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_ALLOC); }
+    if (cudaMemset(h->not_bpsk, 0, 2 * sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_CUDA); }
     if ((rc = build_tables(h)) != PLSPEC_OK) return fail(rc);
     if ((rc = select_kernel(h)) != PLSPEC_OK) return fail(rc);
     *out = h;
@@ -643,7 +654,7 @@ int plspec_finalize(plspec_handle h, float *S_out) {
 int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, int guard, int *k_up, float *p_up,
                    int *k_dn, float *p_dn, float *noise, void *stream) {
     if (!S || !k_up || !p_up || !k_dn || !p_dn || !noise) return PLSPEC_ERR_INVALID_ARG;
-    if (!is_pow2(N) || N < 16 || n_ranges < 1 || n_ipp < 1 || k_min < 1 || k_min >= N / 2 || guard < 0)
+    if (!is_pow2(N) || N < 16 || N > 65536 || n_ranges < 1 || n_ipp < 1 || k_min < 1 || k_min >= N / 2 || guard < 0)
         return PLSPEC_ERR_INVALID_ARG;
     const void *ptrs[] = {S, k_up, p_up, k_dn, p_dn, noise};
     for (const void *p : ptrs) {                         // device (or managed) memory only
@@ -660,7 +671,7 @@ int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, in
 
 int plspec_mean_spectrum(const float *S, float *P_out, int n_ranges, int N, int n_ipp, int centred, void *stream) {
     if (!S || !P_out || S == P_out) return PLSPEC_ERR_INVALID_ARG;
-    if (!is_pow2(N) || N < 16 || n_ranges < 1 || n_ipp < 1 || (centred != 0 && centred != 1))
+    if (!is_pow2(N) || N < 16 || N > 65536 || n_ranges < 1 || n_ipp < 1 || (centred != 0 && centred != 1))
         return PLSPEC_ERR_INVALID_ARG;
     const void *ptrs[] = {S, P_out};
     for (const void *p : ptrs) {                         // device (or managed) memory only, 16-byte aligned
@@ -671,10 +682,50 @@ int plspec_mean_spectrum(const float *S, float *P_out, int n_ranges, int N, int 
     }
     const long long n_vec = (long long)n_ranges * (N / 4);
     long long blocks = (n_vec + 255) / 256;
-    if (blocks > 148 * 8) blocks = 148 * 8;              // grid-stride: eight CTAs of 256 per SM
+    const int n_sm = device_sm_count();
+    if (n_sm < 1) return PLSPEC_ERR_CUDA;
+    if (blocks > n_sm * 8) blocks = n_sm * 8;            // grid-stride: eight CTAs of 256 per SM
     mean_spectrum_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>((const float4 *)S, (float4 *)P_out, n_vec,
                                                                              ilog2(N), n_ipp, centred);
     if (cudaGetLastError() != cudaSuccess) return PLSPEC_ERR_CUDA;
+    return PLSPEC_OK;
+}
+
+int plspec_diag_fp32_peak(int packed, int iters, int reps, double *tflops_best, double *tflops_mean, void *stream_) {
+    if ((packed != 0 && packed != 1) || iters < 1 || reps < 1 || reps > 100000 || !tflops_best || !tflops_mean)
+        return PLSPEC_ERR_INVALID_ARG;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int n_sm = device_sm_count();
+    if (n_sm < 1) return PLSPEC_ERR_CUDA;
+    const unsigned grid = (unsigned)n_sm * 4, block = 512;            // 2048 resident threads per SM
+    float *sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = PLSPEC_OK;
+    if (cudaMalloc((void **)&sink, sizeof(float)) != cudaSuccess) { (void)cudaGetLastError(); return PLSPEC_ERR_ALLOC; }
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) rc = PLSPEC_ERR_CUDA;
+    const double flop = (double)grid * block * (double)iters * 64.0;  // 32 multiply-adds per thread and iteration
+    double best = 0.0, sum = 0.0;
+    for (int r = -1; r < reps && rc == PLSPEC_OK; r++) {              // r = -1: warm-up launch, not counted
+        cudaEventRecord(e0, stream);
+        if (packed) fma_peak_kernel<true><<<grid, block, 0, stream>>>(sink, 0.999f, 0.001f, iters);
+        else        fma_peak_kernel<false><<<grid, block, 0, stream>>>(sink, 0.999f, 0.001f, iters);
+        cudaEventRecord(e1, stream);
+        float ms = 0.f;
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess || ms <= 0.f) {
+            rc = PLSPEC_ERR_CUDA;
+            break;
+        }
+        if (r < 0) continue;
+        const double tf = flop / ((double)ms * 1e-3) / 1e12;
+        if (tf > best) best = tf;
+        sum += tf;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (rc != PLSPEC_OK) { (void)cudaGetLastError(); return rc; }
+    *tflops_best = best;
+    *tflops_mean = sum / reps;
     return PLSPEC_OK;
 }
 

@@ -316,7 +316,12 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     auto pf_base = [&](int t, int pp) {            // this thread's first sample of (tile t, IPP pp)
         const int rr = group_of(t) * G + g;
         const long long off = (long long)P.r0 + (long long)(rr < P.R ? rr : P.R - 1) * P.stride;
-        return reinterpret_cast<const uint32_t *>(P.V) + ((long long)pp * P.v_pitch + off + 64 * wa + lane) * WPS;
+        // Only the +-1 path consumes the prefetched words, and it implies code_len == N: the whole window lies
+        // inside the caller's V.  Any other code may be shorter than N (reading A6), so the window can run past
+        // the end of V: the (unused, but unconditionally issued) loads are then pointed at the twiddle table
+        // twN, which always holds 16384 float2 = one window of either dtype; every lane reads the same words.
+        return bpsk ? reinterpret_cast<const uint32_t *>(P.V) + ((long long)pp * P.v_pitch + off + 64 * wa + lane) * WPS
+                    : reinterpret_cast<const uint32_t *>(P.twN);
     };
     auto pf_load = [&](const uint32_t *b, auto i_) {   // sample i = 2 t_hi + o of the thread's window
         constexpr int i = decltype(i_)::value;

@@ -301,6 +301,35 @@ __global__ void __launch_bounds__(256) mean_spectrum_kernel(const float4 *__rest
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// Diagnostic (SURVEY.md section 7 step 6, 8(d) "measured FMA peak to be reported beside it"): the FP32 FMA issue
+// rate of the device, the measured denominator of the ALU roofline.  Every thread runs 32 independent
+// multiply-add chains -- 32 scalar FFMA, or 16 packed FFMA2 (the form the fused kernel issues) -- per loop
+// iteration: 64 flop per thread and iteration either way.  2048 threads per SM keep every sub-partition's
+// FMA pipe full; nothing touches memory inside the loop.
+template <bool PACKED>
+__global__ void __launch_bounds__(512) fma_peak_kernel(float *__restrict__ out, float a, float b, int iters) {
+    float2 acc[16];
+#pragma unroll
+    for (int j = 0; j < 16; j++) acc[j] = make_float2((float)(threadIdx.x + j), (float)(blockIdx.x - j));
+    const float2 a2 = make_float2(a, a), b2 = make_float2(b, b);
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int j = 0; j < 16; j++) {
+            if constexpr (PACKED) {
+                acc[j] = __ffma2_rn(acc[j], a2, b2);
+            } else {
+                acc[j].x = fmaf(acc[j].x, a, b);
+                acc[j].y = fmaf(acc[j].y, a, b);
+            }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < 16; j++) s += acc[j].x + acc[j].y;
+    if (s == 1.2345678e-30f) out[0] = s;            // never true for the constants used; keeps the chains alive
+}
+
 __device__ __forceinline__ void tile_of_block(const KParams &P, int &r, int &q, int &p_begin, int &p_end) {
     int tile = blockIdx.x;
     r = tile % P.R;

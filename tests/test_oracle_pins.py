@@ -139,6 +139,49 @@ def test_I4_identity_code_is_periodogram():
         assert np.max(np.abs(S[r] - ref)) <= 1e-10 * ref.max()
 
 
+@pytest.mark.parametrize("N,R,r0,s,ipp_len,sc16", [
+    (65536, 3, 0, 4, 131072, False),      # cfg4's geometry: r0, stride, row pitch (BASELINE.json configs[3])
+    (16384, 3, 5, 1, 32768, True),        # cfg3's geometry, sc16 input, a non-zero first sample
+    (8192, 2, 0, 1, 250000, True),        # cfg5's row pitch: offsets p * ipp_len beyond 2^17
+])
+def test_I4_identity_code_is_periodogram_at_the_sizes_the_oracle_judges(N, R, r0, s, ipp_len, sc16):
+    """The oracle is the checker at N = 8192 ... 65536 with large row pitches: pin its twiddle indexing
+    (k * step), bit reversal and p * ipp_len offsets there, against numpy's complex128 FFT.  The last
+    gate is moved to the far end of the row so that a wrong pitch or an int overflow cannot go unseen."""
+    P = 2
+    if sc16:
+        V = rng.integers(-3000, 3000, size=(P, ipp_len, 2)).astype(np.int16)
+        Vc = V[..., 0].astype(np.float64) + 1j * V[..., 1].astype(np.float64)
+    else:
+        V = crandn(P, ipp_len)
+        Vc = V.astype(np.complex128)
+    C = np.ones((P, N), dtype=np.complex64)
+    S = oracle.spectra(V, C, N=N, n_ranges=R, r0=r0, stride=s)
+    far = ipp_len - N                                           # one more gate flush with the end of the row
+    S_far = oracle.spectra(V, C, N=N, n_ranges=1, r0=far, stride=1)
+    for r, off in [(r, r0 + r * s) for r in range(R)] + [(-1, far)]:
+        ref = sum(np.abs(np.fft.fft(Vc[p, off: off + N])) ** 2 for p in range(P))
+        got = S_far[0] if r < 0 else S[r]
+        assert np.max(np.abs(got - ref)) <= 1e-10 * ref.max()
+
+
+def test_I3_tone_closed_form_at_N65536_with_the_chirp_code():
+    """Single tone through cfg4's complex chirp at full length: lands in bin k of the right gate with
+    P A^2 L^2 (conj on the code, forward sign, stride-4 gate indexing), nothing at N - k."""
+    w = synth.CONFIGS["cfg4"]
+    N, P, k, g, A = w.N, 2, 12345, 2, 0.25
+    C = synth.make_codes(synth.scaled(w, n_ranges=1, n_ipp=P), np.random.default_rng(0))
+    assert np.abs(C.imag).max() > 0.5 and np.allclose(np.abs(C), 1.0, atol=1e-6)
+    V = np.zeros((P, w.ipp_len), dtype=np.complex64)
+    d = w.r0 + g * w.stride
+    V[:, d:d + N] = (A * C.astype(np.complex128) * np.exp(2j * np.pi * k * np.arange(N) / N)).astype(np.complex64)
+    S = oracle.spectra(V, C, N=N, n_ranges=4, r0=w.r0, stride=w.stride)
+    expected = P * A * A * N * N
+    assert int(np.argmax(S[g])) == k and abs(S[g, k] - expected) <= 2e-6 * expected
+    assert S[g, N - k] <= 1e-9 * expected
+    assert S[g].sum() - S[g, k] <= 1e-9 * expected * N         # no leakage: L = N, unit-modulus code
+
+
 # ---- I5: zero in, zero out ---------------------------------------------------------------
 def test_I5_zero_input_zero_output():
     C = qpsk(2, 32)
