@@ -64,10 +64,16 @@ enum { PLSPEC_OPT_KERNEL     = 1,   /* [0] 0 = auto, 1 = generic radix-2 kernel,
                                        IPPs batched to fit) and the fused kernel transforms the N/16384 residues
                                        as separate length-16384 windows; 0 = each (gate, residue) CTA decodes the
                                        whole window itself (no scratch, N/16384 times the loads).               */
-       PLSPEC_OPT_SHARED_CODE = 7   /* [0] 1 = `codes` of plspec_accumulate holds ONE code of code_len samples that
+       PLSPEC_OPT_SHARED_CODE = 7,  /* [0] 1 = `codes` of plspec_accumulate holds ONE code of code_len samples that
                                        decodes every IPP of the call (a transmitter that repeats its waveform, e.g.
                                        the chirp of BASELINE config 4); 0 = codes[n_ipp][code_len], one per IPP.
                                                                                             */
+       PLSPEC_OPT_DEFER      = 8    /* [1] host-buffer calls only.  1 = the second half of each call's IPPs is copied
+                                       to the device at once but transformed later: by plspec_finalize, one gate
+                                       range after the other, so that each range's spectra are written out (device
+                                       -> host) while the next range is still being transformed; or, if another
+                                       plspec_accumulate comes first, by that call.  0 = every IPP is transformed
+                                       by the call that brought it.  Results are identical.                       */
      };
 
 /* Counters since create (EXTENSION; used by bench.py for gpu_launches / h2d bytes). */

@@ -30,6 +30,7 @@ PLSPEC_OPT_BPSK_PACK = 4
 PLSPEC_OPT_STAGE = 5
 PLSPEC_OPT_SPLIT = 6
 PLSPEC_OPT_SHARED_CODE = 7
+PLSPEC_OPT_DEFER = 8
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_FUSED = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -201,7 +202,7 @@ class Integrator:
     """Owns one plspec handle.  `accumulate` / `finalize` forward to the C calls."""
 
     def __init__(self, N, code_len, n_ranges, r0=0, stride=1, ipp_len=0, dtype=PLSPEC_CF32,
-                 kernel=KERNEL_AUTO, ipp_chunks=0, h2d_batch=0, bpsk_pack=1, stage=1, split=1, shared_code=0):
+                 kernel=KERNEL_AUTO, ipp_chunks=0, h2d_batch=0, bpsk_pack=1, stage=1, split=1, shared_code=0, defer=1):
         self.N, self.n_ranges = N, n_ranges
         self.h = plspec_create(N, code_len, n_ranges, r0, stride, ipp_len, dtype)
         try:
@@ -219,6 +220,8 @@ class Integrator:
                 plspec_configure(self.h, PLSPEC_OPT_SPLIT, 0)
             if shared_code:
                 plspec_configure(self.h, PLSPEC_OPT_SHARED_CODE, 1)
+            if not defer:
+                plspec_configure(self.h, PLSPEC_OPT_DEFER, 0)
         except Exception:
             self.close()
             raise

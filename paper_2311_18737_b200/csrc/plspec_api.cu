@@ -17,6 +17,8 @@ namespace {
 
 constexpr int kSlots = 3;            // host->device staging ring depth
 constexpr int kMaxNk = 16384;        // largest window one SM holds (fused and generic kernels)
+constexpr int kMaxRanges = 8;        // gate ranges of the overlapped write-out (plspec_finalize to a host buffer)
+constexpr size_t kTailMaxBytes = (size_t)256 << 20;   // device staging of the deferred IPPs of a host-buffer call
 
 struct Slot {
     void   *V = nullptr;             // [batch][span] voltages (storage dtype)
@@ -24,6 +26,37 @@ struct Slot {
     cudaEvent_t ready = nullptr;     // copies into the slot finished   (recorded on copy stream)
     cudaEvent_t freed = nullptr;     // kernel reading the slot finished (recorded on compute stream)
     bool used = false;
+};
+
+// Codes of one launch as the kernels want them: the one code of shared-code mode spread over n_ipp rows, and the
+// bit-packed signs of +-1 codes.  Two instances per handle: the launch in flight, and the deferred tail (below).
+struct CodePrep {
+    float2 *crep = nullptr;          // shared-code mode: [n_ipp][L]
+    long long crep_elems = 0;
+    uint32_t *cbits = nullptr;       // [n_ipp][Q][512] packed code signs (BPSK fast path)
+    long long cbits_words = 0;
+    int flag = 0;                    // index of this instance's word in plspec_ctx::not_bpsk
+    // result of prepare_codes
+    const float2 *C = nullptr;       // codes[n_ipp][L] the kernels read
+    bool packed = false;             // cbits holds this launch's signs; the flag word says whether they apply
+    int epoch = 1;
+};
+
+// Host-buffer calls (a0): the last IPPs of the latest plspec_accumulate are copied to the device but NOT transformed
+// yet.  If plspec_finalize comes next they are transformed one gate range after the other, and each range's spectra
+// are un-permuted and copied out while the next range is still being transformed (the write-out overlaps the
+// compute instead of following it); if another plspec_accumulate comes first they are transformed then, over all
+// gates at once, like every other batch.
+struct Tail {
+    void   *V = nullptr;             // [n_ipp][span]
+    float2 *C = nullptr;             // [n_ipp][L] (one row in shared-code mode)
+    size_t v_bytes = 0, c_bytes = 0; // capacities
+    int n_ipp = 0;
+    bool pending = false;
+    cudaEvent_t ready = nullptr;     // copies landed (copy stream)
+    cudaEvent_t done = nullptr;      // kernels that read the buffers finished
+    bool used = false;
+    CodePrep cp;
 };
 
 }  // namespace
@@ -37,6 +70,7 @@ struct plspec_ctx {
     int Nk = 0, Q = 1, RA = 1;   // N = Q * Nk, Nk = 1024 * RA (fused)
     int gates_per_cta = 1, n_groups = 0;
     int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1, opt_stage = 1, opt_split = 1, opt_shared_code = 0;
+    int opt_defer = 1;
     // split path for N > 16384 (fused kernel only): decode + outer butterfly once into `xq`, then the
     // Q == 1 fused kernel over R * Q virtual gates of length Nk
     bool split = false;
@@ -54,17 +88,18 @@ struct plspec_ctx {
     float  *S = nullptr;             // [R][Q][Nk]
     float  *S_tmp = nullptr;         // un-permute target when S_out is a host pointer
     float2 *twA = nullptr, *twB = nullptr, *twN = nullptr;
-    uint32_t *cbits = nullptr;       // packed code signs of the launch in flight (BPSK fast path)
-    long long cbits_words = 0;
-    int *not_bpsk = nullptr;         // [0]: device flag written by pack_codes_kernel; [1]: never written, always 0
+    CodePrep cp;                     // codes of the launch in flight
+    int *not_bpsk = nullptr;         // device flags written by pack_codes_kernel: [0] cp, [2] tail.cp; [1]: never
+                                     // written, always 0
     int epoch = 0;                   // number of the last code pre-pass
-    float2 *crep = nullptr;          // shared-code mode: the call's one code, one row per IPP
-    long long crep_elems = 0;
     // host pipeline
     cudaStream_t copy_stream = nullptr;
     Slot slot[kSlots];
     int slot_batch = 0;              // IPPs each slot can hold
     int next_slot = 0;
+    Tail tail;
+    cudaStream_t d2h_stream = nullptr;
+    cudaEvent_t range_done[kMaxRanges] = {};
     // ordering
     cudaEvent_t work_done = nullptr;
     cudaStream_t last_stream = nullptr;
@@ -98,14 +133,16 @@ int device_sm_count() {
     return n;
 }
 
-template <int RA, int Q, bool ST>
+template <int RA, int Q, bool ST, bool PFE = true>
 const void *fused_ptr(int dt) {
-    return dt == DT_CF32 ? (const void *)fused_kernel<RA, Q, DT_CF32, ST>
-                         : (const void *)fused_kernel<RA, Q, DT_SC16, ST>;
+    return dt == DT_CF32 ? (const void *)fused_kernel<RA, Q, DT_CF32, ST, PFE>
+                         : (const void *)fused_kernel<RA, Q, DT_SC16, ST, PFE>;
 }
-// the outer radix Q > 1 only occurs with the largest inner size (Nk = 16384, RA = 16)
-const void *fused_lookup(int RA, int Q, int dt, bool st) {
+// the outer radix Q > 1 only occurs with the largest inner size (Nk = 16384, RA = 16).  `prefetch`: the direct-load
+// kernel at Nk = 16384 may fetch the whole next window ahead of time (only safe when code_len == N)
+const void *fused_lookup(int RA, int Q, int dt, bool st, bool prefetch) {
     if (Q == 1) {
+        if (RA == 16 && !st && !prefetch) return fused_ptr<16, 1, false, false>(dt);
         switch (RA) {
             case 1:  return st ? fused_ptr<1, 1, true>(dt) : fused_ptr<1, 1, false>(dt);
             case 2:  return st ? fused_ptr<2, 1, true>(dt) : fused_ptr<2, 1, false>(dt);
@@ -141,10 +178,10 @@ int select_kernel(plspec_ctx *h) {
         h->staged = h->opt_stage && h->Q == 1 && run + 32 <= (long long)kStageMaxBytes &&
                     (h->gates_per_cta > 1 || h->opt_stage == 2);
         if (h->staged) h->smem = (size_t)kStageOff + (size_t)((run + 15) / 16 * 16 + 16);
-        h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged);
+        h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged, h->L == h->N);
         h->split = h->opt_split && h->Q > 1;
         if (h->split) {
-            h->kfunc_split = fused_lookup(16, 1, DT_CF32, false);
+            h->kfunc_split = fused_lookup(16, 1, DT_CF32, false, true);   // scratch windows are whole: Nk samples each
             PL_CUDA(h, cudaFuncSetAttribute(h->kfunc_split, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageOff));
         }
     } else {
@@ -166,26 +203,8 @@ int select_kernel(plspec_ctx *h) {
     return PLSPEC_OK;
 }
 
-// IPP chunks per (gate, q): more CTAs than one wave can hold, whole waves, few flushes.
-int pick_chunks(const plspec_ctx *h, int n_ipp) {
-    if (h->opt_chunks > 0) return h->opt_chunks < n_ipp ? h->opt_chunks : n_ipp;
-    const long long base = (long long)h->n_groups * h->Q;
-    const int slots = h->slots_per_wave;
-    int best = 1;
-    double best_score = -1.0;
-    for (int c = 1; c <= n_ipp && c <= 64; c++) {
-        const long long tiles = base * c;
-        const long long waves = (tiles + slots - 1) / slots;
-        const double eff = (double)tiles / (double)(waves * slots);
-        const double per = (double)n_ipp / c;            // IPPs per chunk; a flush costs ~half a window
-        const double score = eff * per / (per + 0.5);
-        if (score > best_score + 1e-9) { best_score = score; best = c; }
-    }
-    return best;
-}
-
-int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp,
-                 cudaStream_t stream);
+int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp, int g_lo,
+                 int g_cnt, cudaStream_t stream);
 
 // The fused kernel is launched with programmatic stream serialisation: its prologue (TMEM allocation, twiddle
 // tables) overlaps the tail of whatever precedes it in the stream; it calls griddepcontrol.wait before it reads
@@ -212,68 +231,97 @@ __global__ void replicate_code_kernel(const float2 *__restrict__ code, float2 *_
         rows[i] = __ldg(code + (int)(i % L));
 }
 
-int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0,
-                      int n_ipp, cudaStream_t stream) {
+// Step 1 of a launch: bring the codes of n_ipp pulses into the form the kernels read (cp.C, cp.cbits).
+int prepare_codes(plspec_ctx *h, CodePrep &cp, const float2 *dC, int n_ipp, cudaStream_t stream) {
     if (h->opt_shared_code) {
         const long long total = (long long)n_ipp * h->L;
-        if (total > h->crep_elems) {
-            if (h->crep) cudaFree(h->crep);
-            h->crep = nullptr; h->crep_elems = 0;
-            if (cudaMalloc((void **)&h->crep, sizeof(float2) * (size_t)total) != cudaSuccess) {
+        if (total > cp.crep_elems) {
+            if (cp.crep) cudaFree(cp.crep);
+            cp.crep = nullptr; cp.crep_elems = 0;
+            if (cudaMalloc((void **)&cp.crep, sizeof(float2) * (size_t)total) != cudaSuccess) {
                 (void)cudaGetLastError();
                 return PLSPEC_ERR_ALLOC;
             }
-            h->crep_elems = total;
+            cp.crep_elems = total;
         }
-        replicate_code_kernel<<<h->n_sm * 4, 256, 0, stream>>>(dC, h->crep, h->L, total);
+        replicate_code_kernel<<<h->n_sm * 4, 256, 0, stream>>>(dC, cp.crep, h->L, total);
         PL_CUDA(h, cudaGetLastError());
         h->stats.kernel_launches++;
-        dC = h->crep;
+        dC = cp.crep;
     }
-    if (h->kind == 2 && h->split) return launch_split(h, dV, dC, v_pitch, r0, n_ipp, stream);
-    KParams P;
-    P.V = dV; P.C = dC; P.S = h->S; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
-    P.v_pitch = v_pitch;
-    P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
-    P.L = h->L; P.R = h->R; P.r0 = r0; P.stride = h->stride;
-    P.n_groups = h->n_groups;
-    P.n_ipp = n_ipp;
-    P.n_chunks = pick_chunks(h, n_ipp);
-    P.use_atomic = P.n_chunks > 1 ? 1 : 0;
-    P.Cbits = nullptr; P.not_bpsk = nullptr; P.epoch = 1;
-    if (h->kind == 2 && h->opt_bpsk && h->L == h->N) {
+    cp.C = dC;
+    cp.packed = false;
+    cp.epoch = 1;
+    if (h->kind == 2 && !h->split && h->opt_bpsk && h->L == h->N) {
         // code pre-pass: pack the signs of real +-1 codes (1 bit / sample instead of 8 bytes); the fused
         // kernel falls back to the general complex decode when the flag says the codes are anything else
         const long long words = (long long)n_ipp * h->Q * 512;
-        if (words > h->cbits_words) {
-            if (h->cbits) cudaFree(h->cbits);
-            h->cbits = nullptr; h->cbits_words = 0;
-            if (cudaMalloc((void **)&h->cbits, sizeof(uint32_t) * (size_t)words) != cudaSuccess) {
+        if (words > cp.cbits_words) {
+            if (cp.cbits) cudaFree(cp.cbits);
+            cp.cbits = nullptr; cp.cbits_words = 0;
+            if (cudaMalloc((void **)&cp.cbits, sizeof(uint32_t) * (size_t)words) != cudaSuccess) {
                 (void)cudaGetLastError();
                 return PLSPEC_ERR_ALLOC;
             }
-            h->cbits_words = words;
+            cp.cbits_words = words;
         }
         h->epoch = h->epoch == 0x7fffffff ? 1 : h->epoch + 1;
-        P.epoch = h->epoch;
-        pack_codes_kernel<<<(unsigned)((words + 255) / 256), 256, 0, stream>>>(dC, h->cbits, h->not_bpsk, h->epoch, h->L, h->Nk,
-                                                                              h->RA, h->Q, words);
+        cp.epoch = h->epoch;
+        pack_codes_kernel<<<(unsigned)((words + 255) / 256), 256, 0, stream>>>(dC, cp.cbits, h->not_bpsk + cp.flag, cp.epoch,
+                                                                              h->L, h->Nk, h->RA, h->Q, words);
         PL_CUDA(h, cudaGetLastError());
         h->stats.kernel_launches++;
-        P.Cbits = h->cbits; P.not_bpsk = h->not_bpsk;
+        cp.packed = true;
     }
-    long long tiles = (long long)h->n_groups * h->Q * P.n_chunks;
+    return PLSPEC_OK;
+}
+
+// Step 2 of a launch: decode + FFT + power + accumulate of n_ipp pulses for the gates [g_lo, g_lo + g_cnt) into
+// their rows of S_dev.  g_lo is a multiple of the fused kernel's gates per CTA.  r0 = sample of gate 0 in a row of dV.
+int launch_gates(plspec_ctx *h, const CodePrep &cp, const void *dV, long long v_pitch, int r0, int n_ipp, int g_lo, int g_cnt,
+                 cudaStream_t stream) {
+    if (h->kind == 2 && h->split) return launch_split(h, dV, cp.C, v_pitch, r0, n_ipp, g_lo, g_cnt, stream);
+    const int n_groups = (g_cnt + h->gates_per_cta - 1) / h->gates_per_cta;
+    KParams P;
+    P.V = dV; P.C = cp.C; P.S = h->S + (size_t)g_lo * (size_t)h->N;
+    P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
+    P.v_pitch = v_pitch;
+    P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
+    P.L = h->L; P.R = g_cnt; P.r0 = r0 + g_lo * h->stride; P.stride = h->stride;
+    P.n_groups = n_groups;
+    P.n_ipp = n_ipp;
+    P.Cbits = cp.packed ? cp.cbits : nullptr;
+    P.not_bpsk = cp.packed ? h->not_bpsk + cp.flag : nullptr;
+    P.epoch = cp.epoch;
+    long long tiles;
     if (h->kind == 2) {
         // fused kernel: flattened schedule.  auto = one CTA per resident slot, each an equal run of
         // (tile, IPP) items; explicit chunks = that many equal IPP runs per tile, one CTA each
-        const long long items = (long long)h->n_groups * h->Q * n_ipp;
+        const long long items = (long long)n_groups * h->Q * n_ipp;
         if (h->opt_chunks > 0) {
             P.n_chunks = h->opt_chunks < n_ipp ? h->opt_chunks : n_ipp;
-            tiles = (long long)h->n_groups * h->Q * P.n_chunks;
+            tiles = (long long)n_groups * h->Q * P.n_chunks;
         } else {
             P.n_chunks = 0;
             tiles = items < h->slots_per_wave ? items : h->slots_per_wave;
         }
+        P.use_atomic = 1;
+    } else {
+        // generic kernel: one CTA per (gate, residue, IPP chunk); chunks picked for whole waves
+        int c = h->opt_chunks > 0 ? (h->opt_chunks < n_ipp ? h->opt_chunks : n_ipp) : 1;
+        if (h->opt_chunks <= 0) {
+            const long long base = (long long)g_cnt * h->Q;
+            double best_score = -1.0;
+            for (int k = 1; k <= n_ipp && k <= 64; k++) {
+                const long long t = base * k, waves = (t + h->slots_per_wave - 1) / h->slots_per_wave;
+                const double eff = (double)t / (double)(waves * h->slots_per_wave), per = (double)n_ipp / k;
+                const double score = eff * per / (per + 0.5);              // a flush costs ~half a window
+                if (score > best_score + 1e-9) { best_score = score; c = k; }
+            }
+        }
+        P.n_chunks = c;
+        P.use_atomic = c > 1 ? 1 : 0;
+        tiles = (long long)g_cnt * h->Q * c;
     }
     h->stats.ipp_chunks_last = P.n_chunks;
     if (tiles > 0x7fffffffLL) return PLSPEC_ERR_UNSUPPORTED;
@@ -283,44 +331,60 @@ int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long
     return PLSPEC_OK;
 }
 
+int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0,
+                      int n_ipp, cudaStream_t stream) {
+    const int rc = prepare_codes(h, h->cp, dC, n_ipp, stream);
+    if (rc != PLSPEC_OK) return rc;
+    return launch_gates(h, h->cp, dV, v_pitch, r0, n_ipp, 0, h->R, stream);
+}
+
 // N > 16384: predecode_kernel (every window decoded once, outer radix-Q butterfly) -> scratch -> fused
-// kernel with Q = 1 over R * Q virtual gates, in batches of IPPs that fit the scratch buffer.
-int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp,
-                 cudaStream_t stream) {
-    const long long per_ipp = (long long)h->R * h->N;                 // float2 elements of scratch per IPP
+// kernel with Q = 1 over g_cnt * Q virtual gates, in batches of IPPs that fit the scratch buffer.
+int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp, int g_lo,
+                 int g_cnt, cudaStream_t stream) {
+    const long long per_ipp_full = (long long)h->R * h->N;             // float2 elements of scratch per IPP, all gates
+    const long long per_ipp = (long long)g_cnt * h->N;                 // ... of this launch's gates
     if (!h->xq) {
-        long long want = (4LL << 30) / (per_ipp * (long long)sizeof(float2));   // <= 4 GiB
+        long long want = (4LL << 30) / (per_ipp_full * (long long)sizeof(float2));   // <= 4 GiB
         if (want < 1) want = 1;
         if (want > 64) want = 64;
         if (h->opt_batch > 0 && want > h->opt_batch) want = h->opt_batch;
-        while (want >= 1 && cudaMalloc((void **)&h->xq, (size_t)(want * per_ipp) * sizeof(float2)) != cudaSuccess) {
+        while (want >= 1 && cudaMalloc((void **)&h->xq, (size_t)(want * per_ipp_full) * sizeof(float2)) != cudaSuccess) {
             (void)cudaGetLastError();
             h->xq = nullptr;
             want /= 2;
         }
         if (!h->xq) return PLSPEC_ERR_ALLOC;
         h->xq_ipps = want;
-        h->zero_bits_words = want * 512;
+    }
+    long long fit = h->xq_ipps * per_ipp_full / per_ipp;               // IPPs of g_cnt gates the scratch holds
+    if (h->opt_batch > 0 && fit > h->opt_batch) fit = h->opt_batch;
+    if (fit > 65535) fit = 65535;
+    if (fit * 512 > h->zero_bits_words) {
+        if (h->zero_bits) cudaFree(h->zero_bits);
+        h->zero_bits = nullptr;
+        h->zero_bits_words = fit * 512;
         if (cudaMalloc((void **)&h->zero_bits, sizeof(uint32_t) * (size_t)h->zero_bits_words) != cudaSuccess) {
             (void)cudaGetLastError();
+            h->zero_bits_words = 0;
             return PLSPEC_ERR_ALLOC;
         }
         PL_CUDA(h, cudaMemsetAsync(h->zero_bits, 0, sizeof(uint32_t) * (size_t)h->zero_bits_words, stream));
     }
     const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
-    for (int p0 = 0; p0 < n_ipp; p0 += (int)h->xq_ipps) {
-        const int nb = n_ipp - p0 < (int)h->xq_ipps ? n_ipp - p0 : (int)h->xq_ipps;
+    for (int p0 = 0; p0 < n_ipp; p0 += (int)fit) {
+        const int nb = n_ipp - p0 < (int)fit ? n_ipp - p0 : (int)fit;
         KParams P;
         P.V = (const char *)dV + (size_t)p0 * (size_t)v_pitch * esz;
         P.C = dC + (size_t)p0 * h->L;
-        P.S = h->S; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
+        P.S = h->S + (size_t)g_lo * (size_t)h->N; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
         P.Cbits = nullptr; P.not_bpsk = nullptr; P.epoch = 1;
         P.v_pitch = v_pitch;
         P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
-        P.L = h->L; P.R = h->R; P.r0 = r0; P.stride = h->stride;
-        P.n_groups = h->R; P.n_ipp = nb; P.n_chunks = 1; P.use_atomic = 0;
-        if (h->R > 65535 || nb > 65535) return PLSPEC_ERR_UNSUPPORTED;
-        const dim3 blocks((unsigned)(h->Nk / 512), (unsigned)h->R, (unsigned)nb);
+        P.L = h->L; P.R = g_cnt; P.r0 = r0 + g_lo * h->stride; P.stride = h->stride;
+        P.n_groups = g_cnt; P.n_ipp = nb; P.n_chunks = 1; P.use_atomic = 0;
+        if (g_cnt > 65535) return PLSPEC_ERR_UNSUPPORTED;
+        const dim3 blocks((unsigned)(h->Nk / 512), (unsigned)g_cnt, (unsigned)nb);
         const bool sc = h->dtype == PLSPEC_SC16;
         if (h->Q == 2) {
             if (sc) predecode_kernel<2, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq);
@@ -331,15 +395,15 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
         }
         PL_CUDA(h, cudaGetLastError());
         h->stats.kernel_launches++;
-        // step 2: R * Q virtual gates, window = Nk contiguous decoded samples, identity code
+        // step 2: g_cnt * Q virtual gates, window = Nk contiguous decoded samples, identity code
         KParams F = P;
         F.V = h->xq; F.C = dC;
-        // sign-flip decode, no flips.  The flag word is the handle's permanent zero, not the one pack_codes_kernel
-        // writes: an earlier launch of the unsplit path on this handle may have left any epoch in that one.
+        // sign-flip decode, no flips.  The flag word is the handle's permanent zero, not one pack_codes_kernel
+        // writes: an earlier launch of the unsplit path on this handle may have left any epoch in those.
         F.Cbits = h->zero_bits; F.not_bpsk = h->not_bpsk + 1; F.epoch = 1;
         F.v_pitch = per_ipp;
         F.N = h->Nk; F.Q = 1; F.L = h->Nk;
-        F.R = h->R * h->Q; F.r0 = 0; F.stride = h->Nk;
+        F.R = g_cnt * h->Q; F.r0 = 0; F.stride = h->Nk;
         F.n_groups = F.R;
         const long long items = (long long)F.n_groups * nb;
         long long tiles;
@@ -395,40 +459,92 @@ int ensure_slots(plspec_ctx *h, int batch) {
     return PLSPEC_OK;
 }
 
+// copy the needed span of IPPs [p0, p0 + nb) of a host-buffer call, and their codes, on the copy stream
+int copy_ipps(plspec_ctx *h, const void *V, const void *C, int p0, int nb, void *dV, float2 *dC) {
+    const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
+    const char *src = (const char *)V + ((size_t)p0 * h->ipp_len + h->r0) * esz;
+    PL_CUDA(h, cudaMemcpy2DAsync(dV, (size_t)h->span * esz, src, (size_t)h->ipp_len * esz, (size_t)h->span * esz, nb,
+                                 cudaMemcpyHostToDevice, h->copy_stream));
+    const size_t c_off = h->opt_shared_code ? 0 : (size_t)p0 * h->L * sizeof(float2);
+    const size_t c_bytes = (size_t)(h->opt_shared_code ? 1 : nb) * h->L * sizeof(float2);
+    PL_CUDA(h, cudaMemcpyAsync(dC, (const char *)C + c_off, c_bytes, cudaMemcpyHostToDevice, h->copy_stream));
+    h->stats.h2d_bytes += (long long)nb * (long long)h->span * (long long)esz + (long long)c_bytes;
+    return PLSPEC_OK;
+}
+
+// The deferred IPPs (struct Tail) are transformed now, over all gates, on `stream`.
+int flush_tail(plspec_ctx *h, cudaStream_t stream) {
+    Tail &t = h->tail;
+    if (!t.pending) return PLSPEC_OK;
+    t.pending = false;
+    const int rc = launch_gates(h, t.cp, t.V, h->span, 0, t.n_ipp, 0, h->R, stream);   // codes prepared when they were copied
+    if (rc != PLSPEC_OK) return rc;
+    PL_CUDA(h, cudaEventRecord(t.done, stream));
+    t.used = true;
+    return PLSPEC_OK;
+}
+
 // Host-resident inputs: copy only the needed span of each IPP (PAPER.md:149 item 3) in batches
 // on the copy stream, overlapped with the kernels of earlier batches (PAPER.md:149 item 2).
 int accumulate_from_host(plspec_ctx *h, const void *V, const void *C, int n_ipp, cudaStream_t stream) {
     const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
     const size_t per_ipp = (size_t)h->span * esz + (h->opt_shared_code ? 0 : (size_t)h->L * sizeof(float2));
-    // auto: eight batches per call, but none below ~4 MB (each batch pays the launches' fixed cost once)
-    int batch = (n_ipp + 7) / 8;
-    const int min_batch = (int)(((size_t)4 << 20) / per_ipp) + 1;
-    if (batch < min_batch) batch = min_batch;
-    if (h->opt_batch > 0) batch = h->opt_batch;
-    const int cap = (int)((256u << 20) / per_ipp);        // <= 256 MiB per slot
-    if (batch > cap) batch = cap;
-    if (batch < 1) batch = 1;
-    if (batch > n_ipp) batch = n_ipp;
-    int rc = ensure_slots(h, batch);
-    if (rc) return rc;
-    for (int p0 = 0; p0 < n_ipp; p0 += batch) {
-        const int nb = n_ipp - p0 < batch ? n_ipp - p0 : batch;
-        Slot &sl = h->slot[h->next_slot];
-        h->next_slot = (h->next_slot + 1) % kSlots;
-        if (sl.used) PL_CUDA(h, cudaStreamWaitEvent(h->copy_stream, sl.freed, 0));
-        const char *src = (const char *)V + ((size_t)p0 * h->ipp_len + h->r0) * esz;
-        PL_CUDA(h, cudaMemcpy2DAsync(sl.V, (size_t)h->span * esz, src, (size_t)h->ipp_len * esz,
-                                     (size_t)h->span * esz, nb, cudaMemcpyHostToDevice, h->copy_stream));
-        const size_t c_off = h->opt_shared_code ? 0 : (size_t)p0 * h->L * sizeof(float2);
-        const size_t c_bytes = (size_t)(h->opt_shared_code ? 1 : nb) * h->L * sizeof(float2);
-        PL_CUDA(h, cudaMemcpyAsync(sl.C, (const char *)C + c_off, c_bytes, cudaMemcpyHostToDevice, h->copy_stream));
-        h->stats.h2d_bytes += (long long)nb * (long long)h->span * (long long)esz + (long long)c_bytes;
-        PL_CUDA(h, cudaEventRecord(sl.ready, h->copy_stream));
-        PL_CUDA(h, cudaStreamWaitEvent(stream, sl.ready, 0));
-        rc = launch_accumulate(h, sl.V, sl.C, h->span, 0, nb, stream);
-        if (rc) return rc;
-        PL_CUDA(h, cudaEventRecord(sl.freed, stream));
-        sl.used = true;
+    // the second half of the call's IPPs (as far as they fit kTailMaxBytes) is staged but left for plspec_finalize
+    // (or the next plspec_accumulate): see struct Tail
+    int n_tail = h->opt_defer ? n_ipp - n_ipp / 2 : 0;
+    const size_t tail_cap = kTailMaxBytes / per_ipp;
+    if ((size_t)n_tail > tail_cap) n_tail = (int)tail_cap;
+    const int n_head = n_ipp - n_tail;
+    int rc;
+    if (n_head > 0) {
+        // auto: eight batches per call, but none below ~4 MB (each batch pays the launches' fixed cost once)
+        int batch = (n_head + 7) / 8;
+        const int min_batch = (int)(((size_t)4 << 20) / per_ipp) + 1;
+        if (batch < min_batch) batch = min_batch;
+        if (h->opt_batch > 0) batch = h->opt_batch;
+        const int cap = (int)((256u << 20) / per_ipp);        // <= 256 MiB per slot
+        if (batch > cap) batch = cap;
+        if (batch < 1) batch = 1;
+        if (batch > n_head) batch = n_head;
+        if ((rc = ensure_slots(h, batch)) != PLSPEC_OK) return rc;
+        for (int p0 = 0; p0 < n_head; p0 += batch) {
+            const int nb = n_head - p0 < batch ? n_head - p0 : batch;
+            Slot &sl = h->slot[h->next_slot];
+            h->next_slot = (h->next_slot + 1) % kSlots;
+            if (sl.used) PL_CUDA(h, cudaStreamWaitEvent(h->copy_stream, sl.freed, 0));
+            if ((rc = copy_ipps(h, V, C, p0, nb, sl.V, sl.C)) != PLSPEC_OK) return rc;
+            PL_CUDA(h, cudaEventRecord(sl.ready, h->copy_stream));
+            PL_CUDA(h, cudaStreamWaitEvent(stream, sl.ready, 0));
+            rc = launch_accumulate(h, sl.V, sl.C, h->span, 0, nb, stream);
+            if (rc) return rc;
+            PL_CUDA(h, cudaEventRecord(sl.freed, stream));
+            sl.used = true;
+        }
+    }
+    if (n_tail > 0) {
+        Tail &t = h->tail;
+        const size_t v_need = (size_t)n_tail * h->span * esz;
+        const size_t c_need = (size_t)(h->opt_shared_code ? 1 : n_tail) * h->L * sizeof(float2);
+        if (t.used) PL_CUDA(h, cudaStreamWaitEvent(h->copy_stream, t.done, 0));   // kernels of the previous tail
+        if (v_need > t.v_bytes || c_need > t.c_bytes) {
+            if (t.V) cudaFree(t.V);                                // cudaFree waits for the device
+            if (t.C) cudaFree(t.C);
+            t.V = nullptr; t.C = nullptr; t.v_bytes = t.c_bytes = 0;
+            if (cudaMalloc(&t.V, v_need) != cudaSuccess || cudaMalloc((void **)&t.C, c_need) != cudaSuccess) {
+                (void)cudaGetLastError();
+                return PLSPEC_ERR_ALLOC;
+            }
+            t.v_bytes = v_need; t.c_bytes = c_need;
+        }
+        if (!t.ready) PL_CUDA(h, cudaEventCreateWithFlags(&t.ready, cudaEventDisableTiming));
+        if (!t.done) PL_CUDA(h, cudaEventCreateWithFlags(&t.done, cudaEventDisableTiming));
+        if ((rc = copy_ipps(h, V, C, n_head, n_tail, t.V, t.C)) != PLSPEC_OK) return rc;
+        PL_CUDA(h, cudaEventRecord(t.ready, h->copy_stream));
+        PL_CUDA(h, cudaStreamWaitEvent(stream, t.ready, 0));
+        t.cp.flag = 2;
+        if ((rc = prepare_codes(h, t.cp, t.C, n_tail, stream)) != PLSPEC_OK) return rc;   // with the options of this call
+        t.n_ipp = n_tail;
+        t.pending = true;
     }
     return PLSPEC_OK;
 }
@@ -491,9 +607,18 @@ void free_ctx(plspec_ctx *h) {
     if (h->twA) cudaFree(h->twA);
     if (h->twB) cudaFree(h->twB);
     if (h->twN) cudaFree(h->twN);
-    if (h->cbits) cudaFree(h->cbits);
+    for (CodePrep *cp : {&h->cp, &h->tail.cp}) {
+        if (cp->cbits) cudaFree(cp->cbits);
+        if (cp->crep) cudaFree(cp->crep);
+    }
+    if (h->tail.V) cudaFree(h->tail.V);
+    if (h->tail.C) cudaFree(h->tail.C);
+    if (h->tail.ready) cudaEventDestroy(h->tail.ready);
+    if (h->tail.done) cudaEventDestroy(h->tail.done);
+    if (h->d2h_stream) cudaStreamDestroy(h->d2h_stream);
+    for (int k = 0; k < kMaxRanges; k++)
+        if (h->range_done[k]) cudaEventDestroy(h->range_done[k]);
     if (h->xq) cudaFree(h->xq);
-    if (h->crep) cudaFree(h->crep);
     if (h->zero_bits) cudaFree(h->zero_bits);
     if (h->not_bpsk) cudaFree(h->not_bpsk);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
@@ -547,12 +672,18 @@ int plspec_create(int N, int code_len, int n_ranges, int r0, int stride, int ipp
     if (cudaMalloc((void **)&h->S, s_bytes) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_ALLOC); }
     if (cudaMemset(h->S, 0, s_bytes) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_CUDA); }
     if (cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&h->d2h_stream, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->work_done, cudaEventDisableTiming) != cudaSuccess) {
         (void)cudaGetLastError();
         return fail(PLSPEC_ERR_CUDA);
     }
-    if (cudaMalloc((void **)&h->not_bpsk, 2 * sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_ALLOC); }
-    if (cudaMemset(h->not_bpsk, 0, 2 * sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_CUDA); }
+    for (int k = 0; k < kMaxRanges; k++)
+        if (cudaEventCreateWithFlags(&h->range_done[k], cudaEventDisableTiming) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return fail(PLSPEC_ERR_CUDA);
+        }
+    if (cudaMalloc((void **)&h->not_bpsk, 4 * sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_ALLOC); }
+    if (cudaMemset(h->not_bpsk, 0, 4 * sizeof(int)) != cudaSuccess) { (void)cudaGetLastError(); return fail(PLSPEC_ERR_CUDA); }
     if ((rc = build_tables(h)) != PLSPEC_OK) return fail(rc);
     if ((rc = select_kernel(h)) != PLSPEC_OK) return fail(rc);
     *out = h;
@@ -577,6 +708,10 @@ int plspec_configure(plspec_handle h, int option, int value) {
         case PLSPEC_OPT_SHARED_CODE:
             if (value > 1) return PLSPEC_ERR_INVALID_ARG;
             h->opt_shared_code = value;
+            return PLSPEC_OK;
+        case PLSPEC_OPT_DEFER:
+            if (value > 1) return PLSPEC_ERR_INVALID_ARG;
+            h->opt_defer = value;
             return PLSPEC_OK;
         case PLSPEC_OPT_SPLIT: {
             if (value > 1) return PLSPEC_ERR_INVALID_ARG;
@@ -606,6 +741,7 @@ int plspec_accumulate(plspec_handle h, const void *voltages, const void *codes, 
     if ((rc = pointer_is_device(h, codes, &cdev)) != PLSPEC_OK) return rc;
     if (vdev != cdev) return PLSPEC_ERR_INVALID_ARG;
     if ((rc = chain_streams(h, stream)) != PLSPEC_OK) return rc;
+    if ((rc = flush_tail(h, stream)) != PLSPEC_OK) return rc;        // deferred IPPs of the previous call come first
     if (vdev) rc = launch_accumulate(h, voltages, (const float2 *)codes, h->ipp_len, h->r0, n_ipp, stream);
     else      rc = accumulate_from_host(h, voltages, codes, n_ipp, stream);
     if (rc != PLSPEC_OK) return rc;
@@ -619,34 +755,57 @@ int plspec_finalize(plspec_handle h, float *S_out) {
     if ((rc = pointer_is_device(h, S_out, &out_dev)) != PLSPEC_OK) return rc;
     cudaStream_t st = h->last_stream;
     const size_t total = (size_t)h->R * (size_t)h->N;
-    const float *src = h->S;
-    bool zeroed = false;
-    if (h->Q > 1 || h->kind == 2) {                      // S_dev is not in natural bin order
-        float *dst = S_out;
-        if (!out_dev) {
-            if (!h->S_tmp && cudaMalloc((void **)&h->S_tmp, total * sizeof(float)) != cudaSuccess) {
-                (void)cudaGetLastError();
-                return PLSPEC_ERR_ALLOC;
-            }
-            dst = h->S_tmp;
+    const bool permuted = h->Q > 1 || h->kind == 2;       // S_dev is not in natural bin order
+    if (out_dev && (rc = flush_tail(h, st)) != PLSPEC_OK) return rc;
+    if (!out_dev && !h->S_tmp && cudaMalloc((void **)&h->S_tmp, total * sizeof(float)) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return PLSPEC_ERR_ALLOC;
+    }
+    // Gate ranges.  Device S_out: one.  Host S_out: up to kMaxRanges of >= ~8 MB each; range k is transformed (the
+    // deferred IPPs, if any), un-permuted into S_tmp and copied out on the d2h stream while range k + 1 computes.
+    int n_ranges = 1;
+    if (!out_dev) {
+        const size_t want = total * sizeof(float) / ((size_t)8 << 20);
+        n_ranges = want < 1 ? 1 : (want > (size_t)kMaxRanges ? kMaxRanges : (int)want);
+    }
+    const int n_groups = (h->R + h->gates_per_cta - 1) / h->gates_per_cta;
+    if (n_ranges > n_groups) n_ranges = n_groups;
+    Tail &t = h->tail;
+    const bool tail = t.pending;
+    t.pending = false;
+    const int RAe = h->kind == 2 ? h->RA : 1, NC = h->kind == 2 ? 1024 : h->Nk, M = h->Q * RAe;
+    const int TC = 4096 / M < NC ? 4096 / M : NC;
+    for (int k = 0; k < n_ranges; k++) {
+        const int g_lo = (int)((long long)n_groups * k / n_ranges) * h->gates_per_cta;
+        int g_hi = (int)((long long)n_groups * (k + 1) / n_ranges) * h->gates_per_cta;
+        if (g_hi > h->R) g_hi = h->R;
+        const int g_cnt = g_hi - g_lo;
+        const size_t off = (size_t)g_lo * (size_t)h->N, cnt = (size_t)g_cnt * (size_t)h->N;
+        if (tail && (rc = launch_gates(h, t.cp, t.V, h->span, 0, t.n_ipp, g_lo, g_cnt, st)) != PLSPEC_OK) return rc;
+        float *dst = (out_dev ? S_out : h->S_tmp) + off;
+        if (permuted) {
+            // one pass: transposition to natural bin order + zeroing of the accumulators
+            finalize_kernel<<<dim3((unsigned)g_cnt, (unsigned)(NC / TC)), 256, (size_t)TC * (M + 1) * sizeof(float), st>>>(
+                h->S + off, dst, ilog2(h->Q), ilog2(RAe), NC, TC);
+            PL_CUDA(h, cudaGetLastError());
+            h->stats.kernel_launches++;
+        } else {
+            PL_CUDA(h, cudaMemcpyAsync(dst, h->S + off, cnt * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            PL_CUDA(h, cudaMemsetAsync(h->S + off, 0, cnt * sizeof(float), st));
         }
-        // one pass: transposition to natural bin order + zeroing of the accumulators
-        const int RAe = h->kind == 2 ? h->RA : 1, NC = h->kind == 2 ? 1024 : h->Nk, M = h->Q * RAe;
-        int TC = 4096 / M < NC ? 4096 / M : NC;
-        finalize_kernel<<<dim3((unsigned)h->R, (unsigned)(NC / TC)), 256, (size_t)TC * (M + 1) * sizeof(float), st>>>(
-            h->S, dst, ilog2(h->Q), ilog2(RAe), NC, TC);
-        PL_CUDA(h, cudaGetLastError());
-        h->stats.kernel_launches++;
-        src = dst;
-        zeroed = true;
+        if (!out_dev) {
+            PL_CUDA(h, cudaEventRecord(h->range_done[k], st));
+            PL_CUDA(h, cudaStreamWaitEvent(h->d2h_stream, h->range_done[k], 0));
+            PL_CUDA(h, cudaMemcpyAsync(S_out + off, dst, cnt * sizeof(float), cudaMemcpyDeviceToHost, h->d2h_stream));
+            h->stats.d2h_bytes += (long long)(cnt * sizeof(float));
+        }
     }
-    if (src != S_out) {
-        PL_CUDA(h, cudaMemcpyAsync(S_out, src, total * sizeof(float),
-                                   out_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
-        if (!out_dev) h->stats.d2h_bytes += (long long)(total * sizeof(float));
+    if (tail) {
+        PL_CUDA(h, cudaEventRecord(t.done, st));
+        t.used = true;
     }
-    if (!zeroed) PL_CUDA(h, cudaMemsetAsync(h->S, 0, total * sizeof(float), st));
     PL_CUDA(h, cudaStreamSynchronize(st));
+    if (!out_dev) PL_CUDA(h, cudaStreamSynchronize(h->d2h_stream));
     h->have_work = false;
     return PLSPEC_OK;
 }
@@ -732,6 +891,7 @@ int plspec_diag_fp32_peak(int packed, int iters, int reps, double *tflops_best, 
 int plspec_reset(plspec_handle h) {
     if (!h) return PLSPEC_ERR_INVALID_ARG;
     cudaStream_t st = h->last_stream;
+    h->tail.pending = false;                              // deferred IPPs are dropped with the rest
     PL_CUDA(h, cudaMemsetAsync(h->S, 0, sizeof(float) * (size_t)h->R * (size_t)h->N, st));
     PL_CUDA(h, cudaStreamSynchronize(st));
     h->have_work = false;

@@ -30,6 +30,13 @@ struct KParams {
     int n_groups;           // gate groups per launch: ceil(R / gates per CTA)
     int n_ipp, n_chunks;    // IPPs of this launch are split over n_chunks CTAs per (gate, q)
     int use_atomic;         // 1: partial sums meet in S via red.global.add.f32
+    // ring mode of the fused kernel (N > 16384, plspec_fused.cuh): the fields above describe the caller's problem
+    // (V, C, N, Q = N / Nk, L, R real gates, r0, stride); the decoded residues go through `ring`
+    float2 *ring;           // [ring_depth][gridDim.x][Nk] decoded, butterflied windows (stays in L2)
+    int    *ring_flags;     // [2][ring_depth] arrival counters, 128 bytes apart: ready, then done
+    int ring_depth;         // slots
+    int ring_ahead;         // steps a slice is produced ahead of its use
+    int c_pitch;            // samples between successive code rows (0: one code for every IPP)
 };
 
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
@@ -150,6 +157,15 @@ __device__ __forceinline__ void tmem_ld8(uint32_t a, float (&v)[8]) {
 __device__ __forceinline__ void tmem_wait_ld8(float (&v)[8]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;"
                  : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]));
+}
+// ---- cross-CTA hand-over through global memory (ring mode): release / acquire at gpu scope
+__device__ __forceinline__ void red_release_add(int *p, int v) {
+    asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ int ld_acquire(const int *p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
 }
 // Programmatic dependent launch: a kernel launched with the stream-serialisation attribute may start while
 // its predecessor in the stream is still running; it must not touch anything the predecessor (or any earlier

@@ -205,9 +205,29 @@ __device__ __forceinline__ void bfly_dif_halves(float2 &r, float2 &i) {
 // transforming IPP p - 1; pass A then reads shared memory.  The copy starts at the 16-byte boundary at
 // or below the first sample and ends at the one at or above the last (CUDA allocations are 256-byte
 // granular, so the rounded run never leaves the allocation that holds the samples).
-template <int RA, int Q, int DT, bool ST>
+// PFE = false: no prefetch of the next window (below).  The prefetch reads all N samples of a window whatever the
+// code length, so the host selects it only when code_len == N (plspec_api.cu: select_kernel): with a shorter code
+// (zero-pad reading A6) the last windows of V would be read past the end of the caller's buffer.
+//
+// RQ = 2, 4: RING MODE for N = RQ * 16384 (RA = 16, Q = 1, DT = CF32, no stage, no prefetch; VDT = the caller's voltage
+// dtype).  A CTA can hold the accumulators of only one residue q of a window (X[RQ k + q] = DFT_Nk(x_q)[k],
+// plspec_kernels.cuh), yet every residue needs all N decoded samples.  So the grid (cooperative launch, one CTA per SM,
+// gridDim.x a multiple of RQ) works in lockstep: in round k CTA c owns the virtual gate vg = k gridDim.x + c
+// (gate vg / RQ, residue vg % RQ) for all IPPs; a STEP is one IPP of one round.  For step s every CTA decodes its
+// 1 / gridDim.x slice of the inner index m of ALL windows of the round (so the code samples and the overlapping echo
+// samples it needs are shared by the round's gates and stay in L1), applies the outer radix-RQ butterfly and writes
+// the RQ residues into slot s % depth of a ring in global memory that is small enough to stay in L2; it then
+// transforms its own virtual gate's window of step s - ahead.. from the ring like any 16384-point window.  Hand-over:
+// per slot a `ready` counter (one release-add per warp after its stores; consumers acquire-poll until all
+// 16 gridDim.x warps of the step have arrived) and a `done` counter (one add per warp after its last load of the
+// slot; producers wait for it before they overwrite the slot, `depth` steps later).  Counters are monotonic:
+// slot i serves steps i, i + depth, ... and step s completes at (s / depth + 1) * 16 gridDim.x.  A CTA never waits for
+// a step that needs its own later work, so the grid cannot deadlock as long as all CTAs are resident.
+// The decoded windows never reach DRAM: the scratch round trip of the old split path (2 x 21 GB at cfg 4) is gone.
+template <int RA, int Q, int DT, bool ST, bool PFE = true, int RQ = 0, int VDT = DT_CF32>
 __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P) {
     static_assert(!ST || Q == 1, "the staged variant holds one whole window run in shared memory");
+    static_assert(RQ == 0 || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && !PFE), "ring mode: 16384-point complex64 windows");
     constexpr int ESZ = DT == DT_CF32 ? 8 : 4;
     constexpr int NJ = 16 / RA;            // a' values per thread in pass A
     constexpr int G = 16 / RA;             // gates per CTA
@@ -220,13 +240,16 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     // ---- schedule: the launch's work items (tile, IPP), tile = (gate group, q), are numbered tile-major
     // and CTA c takes the contiguous run [c T / n, (c + 1) T / n) of the T = tiles * n_ipp items: equal
     // work for every CTA, accumulators flushed only where the run crosses into another tile.
-    const long long T = (long long)P.n_groups * Q * P.n_ipp;
-    const long long i0 = (long long)blockIdx.x * T / gridDim.x, i1 = ((long long)blockIdx.x + 1) * T / gridDim.x;
+    // (ring mode: n_groups = rounds, every CTA walks all rounds x IPPs)
+    const long long T = RQ ? (long long)P.n_groups * P.n_ipp : (long long)P.n_groups * Q * P.n_ipp;
+    const long long i0 = RQ ? 0 : (long long)blockIdx.x * T / gridDim.x;
+    const long long i1 = RQ ? T : ((long long)blockIdx.x + 1) * T / gridDim.x;
+    const int Rv = RQ ? P.R * RQ : P.R;            // gates the CTAs walk (ring mode: virtual gates)
     if (i0 >= i1) return;                          // uniform for the CTA; nothing allocated yet
     const int tile0 = (int)(i0 / P.n_ipp);
     const int p0 = (int)(i0 - (long long)tile0 * P.n_ipp);
     // tile -> gate group and residue
-    auto group_of = [&](int t) { return Q == 1 ? t : t % P.n_groups; };
+    auto group_of = [&](int t) { return RQ ? t * (int)gridDim.x + (int)blockIdx.x : (Q == 1 ? t : t % P.n_groups); };
     auto resid_of = [&](int t) { return Q == 1 ? 0 : t / P.n_groups; };
 
     // ---- twiddles live in tensor memory: every thread re-reads only constants it wrote itself
@@ -310,18 +333,13 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
 
     // PF: the raw samples (one 32-bit word each) and the code word of the NEXT window are fetched while the last
     // butterfly stage of the current one retires its registers, so no warp sits on L2 latency at the top of a window
-    constexpr bool PF = RA == 16 && Q == 1 && !ST;
+    constexpr bool PF = PFE && RA == 16 && Q == 1 && !ST;
     constexpr int WPS = DT == DT_SC16 ? 1 : 2;     // 32-bit words per sample
     uint32_t raw[PF ? 32 * WPS : 1], cw_pf = 0;
     auto pf_base = [&](int t, int pp) {            // this thread's first sample of (tile t, IPP pp)
         const int rr = group_of(t) * G + g;
         const long long off = (long long)P.r0 + (long long)(rr < P.R ? rr : P.R - 1) * P.stride;
-        // Only the +-1 path consumes the prefetched words, and it implies code_len == N: the whole window lies
-        // inside the caller's V.  Any other code may be shorter than N (reading A6), so the window can run past
-        // the end of V: the (unused, but unconditionally issued) loads are then pointed at the twiddle table
-        // twN, which always holds 16384 float2 = one window of either dtype; every lane reads the same words.
-        return bpsk ? reinterpret_cast<const uint32_t *>(P.V) + ((long long)pp * P.v_pitch + off + 64 * wa + lane) * WPS
-                    : reinterpret_cast<const uint32_t *>(P.twN);
+        return reinterpret_cast<const uint32_t *>(P.V) + ((long long)pp * P.v_pitch + off + 64 * wa + lane) * WPS;
     };
     auto pf_load = [&](const uint32_t *b, auto i_) {   // sample i = 2 t_hi + o of the thread's window
         constexpr int i = decltype(i_)::value;
@@ -341,6 +359,41 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
     }
 
+    // ---- ring mode: producer side and the two hand-over counters per slot
+    const int ringW = 16 * (int)gridDim.x;         // warp arrivals that complete a step
+    auto ring_wait = [&](int slot, int target) {   // slot < depth: ready counters, >= depth: done counters
+        if (lane == 0) {
+            const int *f = P.ring_flags + 32 * slot;
+            while (ld_acquire(f) < target) { }
+        }
+        __syncwarp();
+    };
+    auto ring_produce = [&](long long sp) {        // this CTA's slice of every window of step sp -> ring slot sp % depth
+        if constexpr (RQ > 0) {
+            constexpr int NKc = 1024 * RA;
+            const int kk = (int)(sp / P.n_ipp), pp = (int)(sp - (long long)kk * P.n_ipp);
+            const int GR = (int)gridDim.x / RQ, g_first = kk * GR;
+            const int gr = (P.R - g_first) < GR ? (P.R - g_first) : GR;
+            const int mp0 = (int)(((long long)blockIdx.x * (NKc / 2)) / gridDim.x);
+            const int mp1 = (int)((((long long)blockIdx.x + 1) * (NKc / 2)) / gridDim.x);
+            const int npair = mp1 - mp0, items = gr * npair;
+            const int slot = (int)(sp % P.ring_depth);
+            float2 *base = P.ring + (size_t)slot * gridDim.x * (size_t)NKc;
+            const float2 *Crow = P.C + (long long)pp * P.c_pitch;
+            for (int it = tid; it < items; it += kFusedThreads) {
+                const int tt = it / npair, m = 2 * (mp0 + it - tt * npair);
+                const long long voff = (long long)pp * P.v_pitch + P.r0 + (long long)(g_first + tt) * P.stride;
+                predecode_pair<RQ, VDT>(P.V, voff, Crow, P.L, NKc, P.twN, m,
+                                        reinterpret_cast<float4 *>(base + (size_t)(tt * RQ) * NKc + m));
+            }
+            __syncwarp();
+            if (lane == 0) red_release_add(P.ring_flags + 32 * slot, 1);
+        }
+    };
+    if constexpr (RQ > 0) {
+        for (long long sp = 0; sp < P.ring_ahead && sp < T; sp++) ring_produce(sp);
+    }
+
     int left = (int)(i1 - i0);                     // items still to do, this one included
     int p_lo = p0;
     for (int tile = tile0; left > 0; tile++, p_lo = 0) {                   // the tiles this CTA's run touches
@@ -349,7 +402,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
     const bool more_tiles = left > 0;
     const int gg = group_of(tile), q = resid_of(tile);
     const int r = gg * G + g;
-    const int r_ld = r < P.R ? r : P.R - 1;        // ragged last group: recompute a valid gate, never flush it
+    const int r_ld = r < Rv ? r : Rv - 1;          // ragged last group: recompute a valid gate, never flush it
     const long long gate_off = (long long)P.r0 + (long long)r_ld * P.stride;
     const long long run_off = (long long)P.r0 + (long long)(gg * G) * P.stride;   // first sample of the CTA's run
     float2 accS[8], accC[8];                       // per last-stage butterfly k of pass B2 (bfly_power)
@@ -359,6 +412,21 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         const bool has_next = p + 1 < p_hi || more_tiles;
         const int p_next = p + 1 < p_hi ? p + 1 : 0;
         const int tile_next = p + 1 < p_hi ? tile : tile + 1;
+        long long rs = 0;                                            // ring mode: this step
+        if constexpr (RQ > 0) {
+            rs = (long long)tile * P.n_ipp + p;
+            const long long sp = rs + P.ring_ahead;
+            if (sp < T) {
+                // slot sp % depth last held step sp - depth: every warp of the grid has loaded it
+                if (sp >= P.ring_depth) ring_wait(P.ring_depth + (int)(sp % P.ring_depth), (int)(sp / P.ring_depth) * ringW);
+                ring_produce(sp);
+            }
+            ring_wait((int)(rs % P.ring_depth), (int)(rs / P.ring_depth + 1) * ringW);
+            if (r >= Rv) {                                           // a round with fewer virtual gates than CTAs
+                if (lane == 0) red_release_add(P.ring_flags + 32 * (P.ring_depth + (int)(rs % P.ring_depth)), 1);
+                continue;
+            }
+        }
         const float2 *Crow = P.C + (long long)p * P.L;
         const long long voff = (long long)p * P.v_pitch + gate_off;
         VSrc vs;
@@ -371,7 +439,15 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
         float2 xr[16], xi[16];
         // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
-        if (PF && bpsk) {
+        if constexpr (RQ > 0) {                                      // decoded already: straight from the ring (L2, never L1)
+            const float2 *win = P.ring + ((size_t)(rs % P.ring_depth) * gridDim.x + blockIdx.x) * (size_t)(1024 * RA) + 64 * wa + lane;
+            sfor<0, RA>([&](auto th_) {
+                constexpr int th = decltype(th_)::value;
+                const float2 z0 = __ldcg(win + th * 1024), z1 = __ldcg(win + th * 1024 + 32);
+                xr[th] = make_float2(z0.x, z1.x);
+                xi[th] = make_float2(z0.y, z1.y);
+            });
+        } else if (PF && bpsk) {
             if constexpr (PF) {
                 sfor<0, RA>([&](auto th_) {
                     constexpr int th = decltype(th_)::value;
@@ -428,6 +504,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             constexpr int jj = decltype(jj_)::value;
             dft_packed<RA, jj * RA>(xr, xi);
         });
+        if constexpr (RQ > 0) {                                      // this warp's loads of the slot have all returned
+            __syncwarp();
+            if (lane == 0) red_release_add(P.ring_flags + 32 * (P.ring_depth + (int)(rs % P.ring_depth)), 1);
+        }
         if constexpr (ST) {
             // this warp has consumed its samples of IPP p; the last of the 16 warps starts the copy of IPP p + 1
             __syncwarp();
@@ -554,7 +634,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         });
     }
     // ---- flush: S_dev[r][q][f_hi = wa][e][c = lane]; other CTAs may hold the rest of this tile's IPPs
-    if (r < P.R) {
+    if (r < Rv) {
         float *Srow = P.S + (((long long)r * Q + q) * RA + wa) * 1024 + lane;
         float2 acc[16];                            // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
         sfor<0, 8>([&](auto k_) {

@@ -31,11 +31,16 @@ def to_dev(a):
 
 
 def run_gpu(w, V, C, *, kernel=pl.KERNEL_AUTO, chunks=0, splits=(None,), where="device", batch=0, bpsk_pack=1,
-            stage=1, split=1):
+            stage=1, split=1, defer=1, out="device"):
     """One integration through the C ABI; returns S as float32 numpy [R][N]."""
-    S = torch.full((w.n_ranges, w.N), -1.0, dtype=torch.float32, device="cuda")
+    if out == "device":
+        S = torch.full((w.n_ranges, w.N), -1.0, dtype=torch.float32, device="cuda")
+    else:
+        S = torch.full((w.n_ranges, w.N), -1.0, dtype=torch.float32)
+        if out == "pinned":
+            S = S.pin_memory()
     with pl.Integrator.for_workload(w, kernel=kernel, ipp_chunks=chunks, h2d_batch=batch,
-                                     bpsk_pack=bpsk_pack, stage=stage, split=split) as it:
+                                     bpsk_pack=bpsk_pack, stage=stage, split=split, defer=defer) as it:
         bounds = [0] + [s for s in splits if s is not None] + [w.n_ipp]
         keep = []
         for a, b in zip(bounds[:-1], bounds[1:]):
@@ -115,7 +120,11 @@ def test_cfg5_scaled_stream_from_pinned_host():
     _, _, stats = check(w, V, C, where="pinned", batch=2)
     esz = 4
     assert stats["h2d_bytes"] == w.n_ipp * (w.span * esz + w.code_len * 8)   # span only, not whole IPPs
-    assert stats["kernel_launches"] == 5 * 2 + 1      # 5 staging batches x (code pre-pass + fused) + un-permute
+    # 4 IPPs in 2 staging batches x (code pre-pass + fused); the other 5 deferred to finalize: code pre-pass,
+    # one gate range (S is small) = fused + un-permute
+    assert stats["kernel_launches"] == 2 * 2 + 1 + 2
+    _, _, stats0 = check(w, V, C, where="pinned", batch=2, defer=0)
+    assert stats0["kernel_launches"] == 5 * 2 + 1      # 5 staging batches x (code pre-pass + fused) + un-permute
 
 
 # ---- every FFT length, both kernels, awkward geometry --------------------------------------------
@@ -421,3 +430,79 @@ def test_shard_plans_as_virtual_ranks_on_one_gpu(N, dtype, stage, world):
     S_cat = torch.cat(blocks, dim=0)
     assert S_cat.shape == (R, N)
     assert gate_metric(S_cat.cpu().numpy(), S_ref).max() <= TOL
+
+
+# ---- the deferred tail of host-buffer calls and the overlapped write-out ---------------
+@pytest.mark.parametrize("N,R,dtype,kernel", [(4096, 1101, synth.CF32, pl.KERNEL_AUTO), (2048, 700, synth.SC16, pl.KERNEL_AUTO),
+                                              (65536, 70, synth.CF32, pl.KERNEL_AUTO), (512, 9000, synth.CF32, pl.KERNEL_GENERIC)])
+@pytest.mark.parametrize("out", ["pinned", "pageable", "device"])
+def test_host_calls_defer_half_and_write_out_by_gate_range(N, R, dtype, kernel, out):
+    """S is large enough for several gate ranges (>= 8 MB each) whose boundaries fall inside the gate count; the
+    deferred IPPs are transformed range by range at finalize (host S_out), or flushed by the next accumulate /
+    a finalize to device memory.  Every variant must give the oracle's spectra."""
+    w, V, C = random_case(N, N, R, 1, 1, 5, dtype, complex_code=(N == 65536))
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    for splits in ((None,), (2,)):                                 # one call; two calls (the second flushes the first's tail)
+        S, stats = run_gpu(w, V, C, kernel=kernel, where="pinned", splits=splits, out=out)
+        assert gate_metric(S, S_ref).max() <= TOL
+        assert stats["d2h_bytes"] == (0 if out == "device" else R * N * 4)
+    S0, _ = run_gpu(w, V, C, kernel=kernel, where="pinned", defer=0, out=out)
+    assert gate_metric(S0, S_ref).max() <= TOL
+
+
+def test_deferred_tail_reset_and_mixed_calls():
+    w, V, C = random_case(2048, 2048, 9, 3, 2, 6, synth.SC16, complex_code=False)
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    ref2 = oracle.spectra(V[4:], C[4:], N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    vp = torch.from_numpy(V).pin_memory()
+    cp = torch.from_numpy(C).pin_memory()
+    out = torch.empty((w.n_ranges, w.N), dtype=torch.float32).pin_memory()
+    with pl.Integrator.for_workload(w) as it:
+        it.accumulate(vp[:4], cp[:4], 4)                  # host call: IPPs 2, 3 deferred
+        it.reset()                                        # ... and dropped with the rest
+        it.accumulate(vp[4:], cp[4:], 2)                  # host call: IPP 5 deferred
+        it.finalize(out)
+        assert gate_metric(out.numpy(), ref2).max() <= TOL
+        it.accumulate(vp[:3], cp[:3], 3)                  # host: deferred tail ...
+        it.accumulate(to_dev(V[3:]), to_dev(C[3:]), 3)    # ... flushed by a device-buffer call
+        dev = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+        it.finalize(dev)
+        assert gate_metric(dev.cpu().numpy(), S_ref).max() <= TOL
+        it.finalize(out)                                  # nothing accumulated since
+        assert float(out.abs().max()) == 0.0
+
+
+# ---- no sample outside the caller's buffers reaches a spectrum (compute-sanitizer is closed on this pool) ----------
+@pytest.mark.parametrize("N,L,dtype,stage", [(4096, 4096, synth.CF32, 1), (8192, 8192, synth.SC16, 1), (16384, 16384, synth.SC16, 1),
+                                             (16384, 700, synth.CF32, 1), (16384, 16384, synth.CF32, 2), (65536, 65536 - 3, synth.CF32, 1),
+                                             (2048, 2048, synth.SC16, 2), (256, 200, synth.CF32, 1)])
+def test_poisoned_guard_bands_around_inputs(N, L, dtype, stage):
+    """V and C sit in the middle of device buffers whose every other byte is poison (NaN for float data, +-32767
+    for sc16), rows packed tightly (ipp_len == span) and starting at an odd element, so the 16-byte rounded bulk
+    copies and any read outside [first sample, last sample] that reaches the arithmetic would show: the spectra
+    must still equal the oracle's."""
+    G = max(1, 16384 // max(N, 1024))
+    w, V, C = random_case(N, L, G + 2, 1, 3, 3, dtype, pad=0, complex_code=(dtype == synth.CF32))
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    guard = 70001                                         # elements of poison on either side (odd: misaligned start)
+    if dtype == synth.CF32:
+        vbuf = torch.full((2 * guard + V.size,), float("nan"), dtype=torch.complex64, device="cuda")
+        vbuf[guard:guard + V.size] = torch.from_numpy(V.reshape(-1)).cuda()
+        v = vbuf[guard:guard + V.size].view(V.shape)
+    else:
+        vbuf = torch.full((2 * guard + V.size // 2, 2), 32767, dtype=torch.int16, device="cuda")
+        vbuf[::2] = -32767
+        vbuf[guard:guard + V.size // 2] = torch.from_numpy(V.reshape(-1, 2)).cuda()
+        v = vbuf[guard:guard + V.size // 2].view(V.shape)
+    cbuf = torch.full((2 * guard + C.size,), float("nan"), dtype=torch.complex64, device="cuda")
+    cbuf[guard:guard + C.size] = torch.from_numpy(C.reshape(-1)).cuda()
+    c = cbuf[guard:guard + C.size].view(C.shape)
+    out = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+    kernel = pl.KERNEL_FUSED if N >= 1024 else pl.KERNEL_GENERIC
+    for chunks in (0, 2):
+        with pl.Integrator.for_workload(w, kernel=kernel, stage=stage, ipp_chunks=chunks) as it:
+            it.accumulate(v, c, w.n_ipp)
+            it.finalize(out)
+        S = out.cpu().numpy()
+        assert np.isfinite(S).all()
+        assert gate_metric(S, S_ref).max() <= TOL
