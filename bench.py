@@ -310,7 +310,10 @@ def main():
     ap.add_argument("--shard", default="replicas", choices=["replicas", "ipp", "gates"],
                     help="N > 1: independent integrations (weak scaling, no collective; default), or ONE "
                          "integration sharded by IPP (sum all-reduce of S) / by range gate (all-gather)")
-    ap.add_argument("--split", type=int, default=1, help="N > 16384: 1 decode pre-pass + scratch, 0 fully fused")
+    ap.add_argument("--split", type=int, default=1, help="N > 16384: 1 decode pre-pass + device scratch (default), 2 ring "
+                    "through L2 (one cooperative launch), 0 fully fused")
+    ap.add_argument("--ring-depth", type=int, default=0, help="N > 16384, ring: steps the ring holds (0 = library default)")
+    ap.add_argument("--ring-ahead", type=int, default=0, help="N > 16384, ring: steps decoded ahead (0 = library default)")
     ap.add_argument("--stage", type=int, default=1, help="1 shared-memory voltage stage where gates share samples, 2 wherever it fits, 0 direct loads")
     ap.add_argument("--shared-code", action="store_true",
                     help="workloads whose code repeats every IPP (cfg4's chirp): pass the one code (PLSPEC_OPT_SHARED_CODE)")
@@ -366,7 +369,8 @@ def main():
     S_pin = torch.empty((rows_local, w.N), dtype=torch.float32).pin_memory()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     it = pl.Integrator(w.N, w.code_len, rows_local, r0_local, w.stride, w.ipp_len, w.dtype, kernel=args.kernel,
-                       ipp_chunks=args.chunks, stage=args.stage, split=args.split, shared_code=int(shared_code))
+                       ipp_chunks=args.chunks, stage=args.stage, split=args.split, shared_code=int(shared_code),
+                       ring_depth=args.ring_depth, ring_ahead=args.ring_ahead)
 
     def exchange(S):
         if mode == "ipp":

@@ -59,21 +59,29 @@ enum { PLSPEC_OPT_KERNEL     = 1,   /* [0] 0 = auto, 1 = generic radix-2 kernel,
                                        with bulk asynchronous copies whenever the run of samples one CTA needs
                                        fits (N <= 16384 and, for complex64 input, N <= 8192); 0 = it always
                                        loads voltages straight from global memory.  Results are identical.  */
-       PLSPEC_OPT_SPLIT      = 6,   /* [1] N > 16384 only.  1 = every window is decoded once by a pre-pass kernel (with
-                                       the outer radix-N/16384 butterfly) into a device scratch buffer (<= 4 GiB,
-                                       IPPs batched to fit) and the fused kernel transforms the N/16384 residues
-                                       as separate length-16384 windows; 0 = each (gate, residue) CTA decodes the
-                                       whole window itself (no scratch, N/16384 times the loads).               */
+       PLSPEC_OPT_SPLIT      = 6,   /* [1] N > 16384 only: how the N/16384 residues of a window (each its own
+                                       length-16384 transform, held by its own CTA) get the decoded samples.
+                                       1 = scratch: a pre-pass kernel writes every decoded window (with the outer
+                                       radix-N/16384 butterfly) to a device buffer (<= 4 GiB, IPPs batched to fit),
+                                       the fused kernel reads it back.  2 = ring: one cooperative launch; every CTA
+                                       decodes a slice of all windows of the current step into a ring of
+                                       PLSPEC_OPT_RING_DEPTH steps that stays in L2, and transforms its residue
+                                       from there (no DRAM traffic for the decoded windows; measured slower than 1
+                                       on B200).  0 = each (gate, residue) CTA decodes the whole
+                                       window itself (no scratch, N/16384 times the loads).  Results agree to
+                                       rounding.                                                                 */
        PLSPEC_OPT_SHARED_CODE = 7,  /* [0] 1 = `codes` of plspec_accumulate holds ONE code of code_len samples that
                                        decodes every IPP of the call (a transmitter that repeats its waveform, e.g.
                                        the chirp of BASELINE config 4); 0 = codes[n_ipp][code_len], one per IPP.
                                                                                             */
-       PLSPEC_OPT_DEFER      = 8    /* [1] host-buffer calls only.  1 = the second half of each call's IPPs is copied
+       PLSPEC_OPT_DEFER      = 8,   /* [1] host-buffer calls only.  1 = the second half of each call's IPPs is copied
                                        to the device at once but transformed later: by plspec_finalize, one gate
                                        range after the other, so that each range's spectra are written out (device
                                        -> host) while the next range is still being transformed; or, if another
                                        plspec_accumulate comes first, by that call.  0 = every IPP is transformed
                                        by the call that brought it.  Results are identical.                       */
+       PLSPEC_OPT_RING_DEPTH = 9,   /* [3] 2..16: steps the ring of PLSPEC_OPT_SPLIT = 2 holds (148 x 128 KB each)     */
+       PLSPEC_OPT_RING_AHEAD = 10   /* [2] 1..depth-1: steps a slice is decoded ahead of its use                       */
      };
 
 /* Counters since create (EXTENSION; used by bench.py for gpu_launches / h2d bytes). */

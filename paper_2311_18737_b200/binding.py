@@ -31,6 +31,8 @@ PLSPEC_OPT_STAGE = 5
 PLSPEC_OPT_SPLIT = 6
 PLSPEC_OPT_SHARED_CODE = 7
 PLSPEC_OPT_DEFER = 8
+PLSPEC_OPT_RING_DEPTH = 9
+PLSPEC_OPT_RING_AHEAD = 10
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_FUSED = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -202,7 +204,7 @@ class Integrator:
     """Owns one plspec handle.  `accumulate` / `finalize` forward to the C calls."""
 
     def __init__(self, N, code_len, n_ranges, r0=0, stride=1, ipp_len=0, dtype=PLSPEC_CF32,
-                 kernel=KERNEL_AUTO, ipp_chunks=0, h2d_batch=0, bpsk_pack=1, stage=1, split=1, shared_code=0, defer=1):
+                 kernel=KERNEL_AUTO, ipp_chunks=0, h2d_batch=0, bpsk_pack=1, stage=1, split=1, shared_code=0, defer=1, ring_depth=0, ring_ahead=0):
         self.N, self.n_ranges = N, n_ranges
         self.h = plspec_create(N, code_len, n_ranges, r0, stride, ipp_len, dtype)
         try:
@@ -216,12 +218,16 @@ class Integrator:
                 plspec_configure(self.h, PLSPEC_OPT_BPSK_PACK, 0)
             if stage != 1:
                 plspec_configure(self.h, PLSPEC_OPT_STAGE, stage)
-            if not split:
-                plspec_configure(self.h, PLSPEC_OPT_SPLIT, 0)
+            if split != 1:
+                plspec_configure(self.h, PLSPEC_OPT_SPLIT, split)
             if shared_code:
                 plspec_configure(self.h, PLSPEC_OPT_SHARED_CODE, 1)
             if not defer:
                 plspec_configure(self.h, PLSPEC_OPT_DEFER, 0)
+            if ring_depth:
+                plspec_configure(self.h, PLSPEC_OPT_RING_DEPTH, ring_depth)
+            if ring_ahead:
+                plspec_configure(self.h, PLSPEC_OPT_RING_AHEAD, ring_ahead)
         except Exception:
             self.close()
             raise

@@ -71,8 +71,16 @@ struct plspec_ctx {
     int gates_per_cta = 1, n_groups = 0;
     int opt_kernel = 0, opt_chunks = 0, opt_batch = 0, opt_bpsk = 1, opt_stage = 1, opt_split = 1, opt_shared_code = 0;
     int opt_defer = 1;
-    // split path for N > 16384 (fused kernel only): decode + outer butterfly once into `xq`, then the
-    // Q == 1 fused kernel over R * Q virtual gates of length Nk
+    // N > 16384, ring mode (PLSPEC_OPT_SPLIT = 2, fused kernel only): one cooperative launch of the Q == 1 fused kernel whose CTAs
+    // decode + butterfly every window once into a ring that stays in L2 and transform it from there
+    bool ring_mode = false;
+    const void *kfunc_ring = nullptr;    // fused_kernel<16, 1, CF32, false, true, Q, dtype>
+    float2 *ring = nullptr;              // [ring_depth][ring_ctas][Nk]
+    int *ring_flags = nullptr;           // [2][ring_depth] x 32 ints
+    int ring_depth = 0, ring_ctas = 0;   // as allocated
+    int opt_ring_depth = 3, opt_ring_ahead = 2;
+    // split path for N > 16384 (PLSPEC_OPT_SPLIT = 1, the default): decode + outer butterfly once into `xq` (device scratch), then
+    // the Q == 1 fused kernel over R * Q virtual gates of length Nk
     bool split = false;
     const void *kfunc_split = nullptr;   // fused_kernel<16, 1, CF32, false>
     float2 *xq = nullptr;                // [batch][R][Q][Nk]
@@ -179,7 +187,18 @@ int select_kernel(plspec_ctx *h) {
                     (h->gates_per_cta > 1 || h->opt_stage == 2);
         if (h->staged) h->smem = (size_t)kStageOff + (size_t)((run + 15) / 16 * 16 + 16);
         h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged, h->L == h->N);
-        h->split = h->opt_split && h->Q > 1;
+        h->split = h->opt_split == 1 && h->Q > 1;
+        h->ring_mode = h->opt_split == 2 && h->Q > 1;
+        if (h->ring_mode) {
+            h->kfunc_ring = h->Q == 2 ? (dt == DT_CF32 ? (const void *)fused_kernel<16, 1, DT_CF32, false, true, 2, DT_CF32>
+                                                       : (const void *)fused_kernel<16, 1, DT_CF32, false, true, 2, DT_SC16>)
+                                      : (dt == DT_CF32 ? (const void *)fused_kernel<16, 1, DT_CF32, false, true, 4, DT_CF32>
+                                                       : (const void *)fused_kernel<16, 1, DT_CF32, false, true, 4, DT_SC16>);
+            PL_CUDA(h, cudaFuncSetAttribute(h->kfunc_ring, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax));
+            int occ_ring = 0;
+            PL_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_ring, h->kfunc_ring, kFusedThreads, (size_t)kStageOff));
+            if (occ_ring < 1) return PLSPEC_ERR_UNSUPPORTED;
+        }
         if (h->split) {
             h->kfunc_split = fused_lookup(16, 1, DT_CF32, false, true);   // scratch windows are whole: Nk samples each
             PL_CUDA(h, cudaFuncSetAttribute(h->kfunc_split, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageOff));
@@ -187,6 +206,7 @@ int select_kernel(plspec_ctx *h) {
     } else {
         h->RA = 0;
         h->split = false;
+        h->ring_mode = false;
         h->gates_per_cta = 1;
         h->block = h->Nk / 2 < 32 ? 32 : (h->Nk / 2 > 512 ? 512 : h->Nk / 2);
         h->smem = (size_t)h->Nk * (sizeof(float2) + sizeof(float));
@@ -205,6 +225,8 @@ int select_kernel(plspec_ctx *h) {
 
 int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp, int g_lo,
                  int g_cnt, cudaStream_t stream);
+int launch_ring(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp, int g_lo,
+                int g_cnt, cudaStream_t stream);
 
 // The fused kernel is launched with programmatic stream serialisation: its prologue (TMEM allocation, twiddle
 // tables) overlaps the tail of whatever precedes it in the stream; it calls griddepcontrol.wait before it reads
@@ -233,6 +255,10 @@ __global__ void replicate_code_kernel(const float2 *__restrict__ code, float2 *_
 
 // Step 1 of a launch: bring the codes of n_ipp pulses into the form the kernels read (cp.C, cp.cbits).
 int prepare_codes(plspec_ctx *h, CodePrep &cp, const float2 *dC, int n_ipp, cudaStream_t stream) {
+    if (h->kind == 2 && h->ring_mode) {                  // the ring kernel reads the codes as given (row pitch 0 or L)
+        cp.C = dC; cp.packed = false; cp.epoch = 1;
+        return PLSPEC_OK;
+    }
     if (h->opt_shared_code) {
         const long long total = (long long)n_ipp * h->L;
         if (total > cp.crep_elems) {
@@ -280,6 +306,7 @@ int prepare_codes(plspec_ctx *h, CodePrep &cp, const float2 *dC, int n_ipp, cuda
 // their rows of S_dev.  g_lo is a multiple of the fused kernel's gates per CTA.  r0 = sample of gate 0 in a row of dV.
 int launch_gates(plspec_ctx *h, const CodePrep &cp, const void *dV, long long v_pitch, int r0, int n_ipp, int g_lo, int g_cnt,
                  cudaStream_t stream) {
+    if (h->kind == 2 && h->ring_mode) return launch_ring(h, dV, cp.C, v_pitch, r0, n_ipp, g_lo, g_cnt, stream);
     if (h->kind == 2 && h->split) return launch_split(h, dV, cp.C, v_pitch, r0, n_ipp, g_lo, g_cnt, stream);
     const int n_groups = (g_cnt + h->gates_per_cta - 1) / h->gates_per_cta;
     KParams P;
@@ -338,7 +365,76 @@ int launch_accumulate(plspec_ctx *h, const void *dV, const float2 *dC, long long
     return launch_gates(h, h->cp, dV, v_pitch, r0, n_ipp, 0, h->R, stream);
 }
 
-// N > 16384: predecode_kernel (every window decoded once, outer radix-Q butterfly) -> scratch -> fused
+// N > 16384, ring mode (plspec_fused.cuh): ONE cooperative launch per <= 2^20 steps.  gridDim.x = the largest
+// multiple of Q that is resident at once (and no more than the launch has virtual gates); round k gives CTA c the
+// virtual gate k gridDim.x + c; the ring holds `depth` steps of gridDim.x residues (depth x 148 x 128 KB = 76 MB at
+// depth 4: inside the 126 MB L2 together with the voltages the producers read).
+int launch_ring(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp, int g_lo,
+                int g_cnt, cudaStream_t stream) {
+    const int Q = h->Q;
+    const int cta_max = (h->n_sm / Q) * Q;
+    if (cta_max < Q) return PLSPEC_ERR_UNSUPPORTED;
+    const int depth = h->opt_ring_depth, ahead = h->opt_ring_ahead < depth ? h->opt_ring_ahead : depth - 1;
+    if (!h->ring || h->ring_depth != depth || h->ring_ctas != cta_max) {
+        if (h->ring) cudaFree(h->ring);                   // waits for the device
+        if (h->ring_flags) cudaFree(h->ring_flags);
+        h->ring = nullptr; h->ring_flags = nullptr; h->ring_depth = 0;
+        if (cudaMalloc((void **)&h->ring, (size_t)depth * cta_max * (size_t)h->Nk * sizeof(float2)) != cudaSuccess ||
+            cudaMalloc((void **)&h->ring_flags, (size_t)(2 * depth + 1) * 32 * sizeof(int)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return PLSPEC_ERR_ALLOC;
+        }
+        PL_CUDA(h, cudaMemsetAsync(h->ring_flags + 64 * depth, 0, sizeof(int), stream));   // error word (see finalize)
+        h->ring_depth = depth; h->ring_ctas = cta_max;
+    }
+    long long vg = (long long)g_cnt * Q;
+    const int n_cta = vg < cta_max ? (int)vg : cta_max;   // a multiple of Q either way
+    const int GR = n_cta / Q, rounds = (g_cnt + GR - 1) / GR;
+    // producer inputs through shared memory if two buffers + the slice's twiddles fit beside the exchange regions
+    // (same arithmetic as the kernel: plspec_fused.cuh, ring mode)
+    const long long vesz = h->dtype == PLSPEC_SC16 ? 4 : 8;
+    const long long npmax = (h->Nk / 2 + n_cta - 1) / n_cta;
+    const long long rcp = 2 * npmax + 2, rvb = (((long long)(GR - 1) * h->stride + 2 * npmax) * vesz + 31) & ~15LL;
+    const long long stage_bytes = 2 * Q * (rcp * 8 + rvb) + (long long)(Q - 1) * 2 * npmax * 8;
+    const int staged = h->opt_stage && stage_bytes <= (long long)kStageMaxBytes ? 1 : 0;
+    const size_t smem = (size_t)kStageOff + (staged ? (size_t)stage_bytes : 0);
+    int per_launch = (1 << 20) / rounds;                  // IPPs per launch: counters stay far below 2^31
+    if (per_launch < 1) return PLSPEC_ERR_UNSUPPORTED;
+    const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
+    const int c_pitch = h->opt_shared_code ? 0 : h->L;
+    for (int p0 = 0; p0 < n_ipp; p0 += per_launch) {
+        const int nb = n_ipp - p0 < per_launch ? n_ipp - p0 : per_launch;
+        PL_CUDA(h, cudaMemsetAsync(h->ring_flags, 0, (size_t)2 * depth * 32 * sizeof(int), stream));
+        KParams P;
+        P.V = (const char *)dV + (size_t)p0 * (size_t)v_pitch * esz;
+        P.C = dC + (size_t)p0 * (size_t)c_pitch;
+        P.S = h->S + (size_t)g_lo * (size_t)h->N; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
+        P.Cbits = nullptr; P.not_bpsk = nullptr; P.epoch = 1;
+        P.v_pitch = v_pitch;
+        P.N = h->N; P.Nk = h->Nk; P.Q = Q; P.log2Nk = ilog2(h->Nk);
+        P.L = h->L; P.R = g_cnt; P.r0 = r0 + g_lo * h->stride; P.stride = h->stride;
+        P.n_groups = rounds; P.n_ipp = nb; P.n_chunks = 0; P.use_atomic = 1;
+        P.ring = h->ring; P.ring_flags = h->ring_flags; P.ring_depth = depth; P.ring_ahead = ahead; P.c_pitch = c_pitch;
+        P.ring_stage = staged;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)n_cta);
+        cfg.blockDim = dim3(kFusedThreads);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeCooperative;      // the CTAs wait on one another: all must be resident
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        void *args[] = {&P};
+        PL_CUDA(h, cudaLaunchKernelExC(&cfg, h->kfunc_ring, args));
+        h->stats.kernel_launches++;
+        h->stats.ipp_chunks_last = 0;
+    }
+    return PLSPEC_OK;
+}
+
+// N > 16384, PLSPEC_OPT_SPLIT = 1 (default): predecode_kernel (every window decoded once, outer radix-Q butterfly) -> scratch -> fused
 // kernel with Q = 1 over g_cnt * Q virtual gates, in batches of IPPs that fit the scratch buffer.
 int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pitch, int r0, int n_ipp, int g_lo,
                  int g_cnt, cudaStream_t stream) {
@@ -619,6 +715,8 @@ void free_ctx(plspec_ctx *h) {
     for (int k = 0; k < kMaxRanges; k++)
         if (h->range_done[k]) cudaEventDestroy(h->range_done[k]);
     if (h->xq) cudaFree(h->xq);
+    if (h->ring) cudaFree(h->ring);
+    if (h->ring_flags) cudaFree(h->ring_flags);
     if (h->zero_bits) cudaFree(h->zero_bits);
     if (h->not_bpsk) cudaFree(h->not_bpsk);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
@@ -713,8 +811,17 @@ int plspec_configure(plspec_handle h, int option, int value) {
             if (value > 1) return PLSPEC_ERR_INVALID_ARG;
             h->opt_defer = value;
             return PLSPEC_OK;
+        case PLSPEC_OPT_RING_DEPTH:
+            if (value < 2 || value > 16) return PLSPEC_ERR_INVALID_ARG;
+            h->opt_ring_depth = value;
+            if (h->opt_ring_ahead >= value) h->opt_ring_ahead = value - 1;
+            return PLSPEC_OK;
+        case PLSPEC_OPT_RING_AHEAD:
+            if (value < 1 || value >= h->opt_ring_depth) return PLSPEC_ERR_INVALID_ARG;
+            h->opt_ring_ahead = value;
+            return PLSPEC_OK;
         case PLSPEC_OPT_SPLIT: {
-            if (value > 1) return PLSPEC_ERR_INVALID_ARG;
+            if (value > 2) return PLSPEC_ERR_INVALID_ARG;
             if (h->have_work) return PLSPEC_ERR_INVALID_ARG;
             h->opt_split = value;
             return select_kernel(h);
@@ -807,6 +914,15 @@ int plspec_finalize(plspec_handle h, float *S_out) {
     PL_CUDA(h, cudaStreamSynchronize(st));
     if (!out_dev) PL_CUDA(h, cudaStreamSynchronize(h->d2h_stream));
     h->have_work = false;
+    if (h->ring_flags) {                                  // a ring-mode wait gave up: the spectra are not to be trusted
+        int err = 0;
+        PL_CUDA(h, cudaMemcpy(&err, h->ring_flags + 64 * h->ring_depth, sizeof(int), cudaMemcpyDeviceToHost));
+        if (err) {
+            (void)cudaMemset(h->ring_flags + 64 * h->ring_depth, 0, sizeof(int));
+            h->last_cuda = (int)cudaErrorLaunchTimeout;
+            return PLSPEC_ERR_CUDA;
+        }
+    }
     return PLSPEC_OK;
 }
 

@@ -37,6 +37,7 @@ struct KParams {
     int ring_depth;         // slots
     int ring_ahead;         // steps a slice is produced ahead of its use
     int c_pitch;            // samples between successive code rows (0: one code for every IPP)
+    int ring_stage;         // 1: the producers' inputs go through shared memory (bulk copies one step ahead)
 };
 
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
@@ -166,6 +167,25 @@ __device__ __forceinline__ int ld_acquire(const int *p) {
     int v;
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
+}
+// ... and inside the CTA (shared memory, cta scope): arrival counting and a published progress word
+__device__ __forceinline__ int atom_add_acq_rel_cta(uint32_t saddr, int v) {
+    int old;
+    asm volatile("atom.acq_rel.cta.shared::cta.add.s32 %0, [%1], %2;" : "=r"(old) : "r"(saddr), "r"(v) : "memory");
+    return old;
+}
+__device__ __forceinline__ int atom_cas_acquire_cta(uint32_t saddr, int cmp, int v) {
+    int old;
+    asm volatile("atom.acquire.cta.shared::cta.cas.b32 %0, [%1], %2, %3;" : "=r"(old) : "r"(saddr), "r"(cmp), "r"(v) : "memory");
+    return old;
+}
+__device__ __forceinline__ int ld_acquire_cta(uint32_t saddr) {
+    int v;
+    asm volatile("ld.acquire.cta.shared::cta.s32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_cta(uint32_t saddr, int v) {
+    asm volatile("st.release.cta.shared::cta.s32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
 }
 // Programmatic dependent launch: a kernel launched with the stream-serialisation attribute may start while
 // its predecessor in the stream is still running; it must not touch anything the predecessor (or any earlier

@@ -38,11 +38,14 @@ constexpr int kRegionBytes = 16 * 65 * 8;                    // 8320
 constexpr int kFusedSmemBytes = 16 * kRegionBytes;
 // control words: stage mbarrier (8) + warp arrival counter (4) + TMEM base (4) + per region a "free" and a
 // "full" mbarrier
-constexpr int kStageCtlBytes = 16 + 32 * 8;
+// + ring mode: per-CTA arrival counters (ready x 4, done x 4), progress words (ready, free) and their poller locks
+constexpr int kRingCtlOff = 16 + 32 * 8;
+constexpr int kStageCtlBytes = kRingCtlOff + 64;
 constexpr int kStageOff = kFusedSmemBytes + kStageCtlBytes;    // voltage stage of the ST variant (16-byte aligned)
 constexpr int kSmemMax = 227 * 1024;
 constexpr int kStageMaxBytes = kSmemMax - kStageOff;
 constexpr int kFusedThreads = 512;
+constexpr int kRingFlushEvery = 10;
 
 // ---- compile-time cos / sin of 2 pi k / 32 (float64, correctly rounded literals)
 constexpr double kCos32d[9] = {1.0,
@@ -200,6 +203,231 @@ __device__ __forceinline__ void bfly_dif_halves(float2 &r, float2 &i) {
 }
 
 // ------------------------------------------------------------------------------------------
+// Ring mode (fused_kernel with RQ = 2, 4; see there), producer side.  These are real functions (not inlined): their
+// working set must not compete with the register allocation of the transform loop that calls them.
+//
+// Producer inputs through shared memory (P.ring_stage != 0: they fit): the code samples and the run of echo samples
+// this CTA's slice needs for step sp are brought in by bulk asynchronous copies (TMA) two steps ahead, into buffer
+// sp & 1, so that the decode reads shared memory instead of waiting on L2; its outer twiddles, which never change
+// (the slice of m is fixed), are loaded once.  Layout per buffer: RQ code rows of `cp` float2, then RQ echo rows of
+// `vb` bytes; every row starts at the 16-byte boundary at or below its first element (as in the ST variant).
+template <int RQ, int VDT>
+struct RingGeo {
+    static constexpr int NK = 16384, VESZ = VDT == DT_CF32 ? 8 : 4;
+    int mp0, npair, npmax, GR, cp, vb, buf;
+    unsigned char *stage;
+    float2 *tws;                                   // [RQ - 1][2 npmax]
+    uint32_t ctl;                                  // ring control words (shared-memory address)
+    __device__ __forceinline__ RingGeo(const KParams *P, unsigned char *smem) {
+        mp0 = (int)(((long long)blockIdx.x * (NK / 2)) / gridDim.x);
+        npair = (int)((((long long)blockIdx.x + 1) * (NK / 2)) / gridDim.x) - mp0;
+        npmax = (NK / 2 + (int)gridDim.x - 1) / (int)gridDim.x;
+        GR = (int)gridDim.x / RQ;
+        cp = 2 * npmax + 2;
+        vb = (((GR - 1) * P->stride + 2 * npmax) * VESZ + 31) & ~15;
+        buf = RQ * (cp * 8 + vb);
+        stage = smem + kStageOff;
+        tws = reinterpret_cast<float2 *>(stage + 2 * buf);
+        ctl = smem_u32(smem + kFusedSmemBytes + kRingCtlOff);
+    }
+};
+
+// one thread: the bulk copies of step sp into buffer sp & 1, counted on that buffer's mbarrier
+template <int RQ, int VDT>
+__device__ __noinline__ void ring_stage_issue_fn(const KParams *P, int sp) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const RingGeo<RQ, VDT> G(P, smem);
+    constexpr int VESZ = RingGeo<RQ, VDT>::VESZ, NK = RingGeo<RQ, VDT>::NK;
+    const uint32_t mb = G.ctl + 48 + 8 * (uint32_t)(sp & 1);
+    const int kk = sp / P->n_ipp, pp = sp - kk * P->n_ipp;
+    const int g_first = kk * G.GR;
+    const int gr = (P->R - g_first) < G.GR ? (P->R - g_first) : G.GR;
+    const unsigned char *cs[RQ], *vs[RQ];
+    uint32_t cb[RQ], vbytes[RQ], total = 0;
+#pragma unroll
+    for (int j = 0; j < RQ; j++) {
+        const int t0 = 2 * G.mp0 + j * NK;
+        int valid = P->L - t0;
+        valid = valid < 0 ? 0 : (valid > 2 * G.npair ? 2 * G.npair : valid);
+        const unsigned char *c = reinterpret_cast<const unsigned char *>(P->C + (long long)pp * P->c_pitch + t0);
+        const unsigned char *v = reinterpret_cast<const unsigned char *>(P->V) +
+                                 ((long long)pp * P->v_pitch + P->r0 + (long long)g_first * P->stride + t0) * VESZ;
+        const uint32_t cm = (uint32_t)(reinterpret_cast<uintptr_t>(c) & 15), vm = (uint32_t)(reinterpret_cast<uintptr_t>(v) & 15);
+        cs[j] = c - cm; vs[j] = v - vm;
+        cb[j] = valid ? ((cm + (uint32_t)valid * 8 + 15u) & ~15u) : 0u;
+        vbytes[j] = valid ? ((vm + (uint32_t)((gr - 1) * P->stride + valid) * VESZ + 15u) & ~15u) : 0u;
+        total += cb[j] + vbytes[j];
+    }
+    mbar_arrive_expect_tx(mb, total);
+    unsigned char *buf = G.stage + (sp & 1) * G.buf;
+#pragma unroll
+    for (int j = 0; j < RQ; j++) {
+        if (cb[j]) bulk_g2s(smem_u32(buf + j * G.cp * 8), cs[j], cb[j], mb);
+        if (vbytes[j]) bulk_g2s(smem_u32(buf + RQ * G.cp * 8 + j * G.vb), vs[j], vbytes[j], mb);
+    }
+}
+
+// whole CTA, once: the slice's outer twiddles W_N^{m q}, and the copies of the first two steps
+template <int RQ, int VDT>
+__device__ __noinline__ void ring_stage_prologue_fn(const KParams *P, int T) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const RingGeo<RQ, VDT> G(P, smem);
+    for (int i = threadIdx.x; i < (RQ - 1) * 2 * G.npair; i += kFusedThreads) {
+        const int q = i / (2 * G.npair) + 1, mm = i - (q - 1) * 2 * G.npair;
+        G.tws[(q - 1) * 2 * G.npmax + mm] = __ldg(P->twN + q * (2 * G.mp0 + mm));
+    }
+    if (threadIdx.x == 0) {
+        fence_proxy_async();
+        ring_stage_issue_fn<RQ, VDT>(P, 0);
+        if (T > 1) ring_stage_issue_fn<RQ, VDT>(P, 1);
+    }
+}
+
+// every warp: this CTA's slice of every window of step sp -> ring slot sp % depth (decode, + outer
+// radix-RQ butterfly, plspec_kernels.cuh).  thread <-> (pair of inner indices, set of gates): the code samples and
+// twiddles of a pair are read once and serve all the thread's gates.  part 0: the thread's first two gates, 1: the
+// rest, -1: all.
+template <int RQ, int VDT>
+__device__ __noinline__ void ring_produce_fn(const KParams *P, int sp, int part) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const RingGeo<RQ, VDT> G(P, smem);
+    constexpr int VESZ = RingGeo<RQ, VDT>::VESZ, NKc = RingGeo<RQ, VDT>::NK;
+    const int tid = threadIdx.x;
+    const bool staged = P->ring_stage != 0;
+    const int L = P->L, stride = P->stride;
+    const int kk = sp / P->n_ipp, pp = sp - kk * P->n_ipp;
+    const int g_first = kk * G.GR;
+    const int gr = (P->R - g_first) < G.GR ? (P->R - g_first) : G.GR;
+    const int npair = G.npair, mp0 = G.mp0;
+    const int lanes_m = npair < kFusedThreads ? npair : kFusedThreads;
+    const int ngs = kFusedThreads / lanes_m;
+    const int my_gs = tid / lanes_m, my_m = tid - my_gs * lanes_m;
+    float2 *base = P->ring + (size_t)(sp % P->ring_depth) * gridDim.x * (size_t)NKc;
+    const float2 *Crow = P->C + (long long)pp * P->c_pitch;
+    const long long vrow = (long long)pp * P->v_pitch + P->r0;
+    const unsigned char *sbuf = G.stage + (sp & 1) * G.buf;
+    int cmis[RQ], vmis[RQ];
+    if (staged) {                                  // wait for this step's copies; element index of sample (m - 2 mp0) in row j = mis_j + ...
+        mbar_wait(G.ctl + 48 + 8 * (uint32_t)(sp & 1), (uint32_t)(sp >> 1) & 1u);
+#pragma unroll
+        for (int j = 0; j < RQ; j++) {
+            const int t0 = 2 * mp0 + j * NKc;
+            cmis[j] = (int)((reinterpret_cast<uintptr_t>(Crow + t0) & 15) >> 3);
+            vmis[j] = (int)((reinterpret_cast<uintptr_t>(reinterpret_cast<const unsigned char *>(P->V) +
+                                                        (vrow + (long long)g_first * stride + t0) * VESZ) & 15) / VESZ);
+        }
+    }
+    if (my_gs >= ngs) return;
+    for (int mp = my_m; mp < npair; mp += lanes_m) {
+        const int m = 2 * (mp0 + mp);
+        float2 c[RQ][2], tw[RQ - 1][2];
+#pragma unroll
+        for (int j = 0; j < RQ; j++)
+#pragma unroll
+            for (int k = 0; k < 2; k++) {
+                const int t = m + k + j * NKc;
+                if (staged)
+                    c[j][k] = t < L ? reinterpret_cast<const float2 *>(sbuf + j * G.cp * 8)[cmis[j] + 2 * mp + k] : make_float2(0.f, 0.f);
+                else
+                    c[j][k] = t < L ? __ldg(Crow + t) : make_float2(0.f, 0.f);
+            }
+        if (staged) {
+#pragma unroll
+            for (int q = 1; q < RQ; q++)
+#pragma unroll
+                for (int k = 0; k < 2; k++) tw[q - 1][k] = G.tws[(q - 1) * 2 * G.npmax + 2 * mp + k];
+        } else {
+            predecode_twiddles<RQ>(P->twN, m, tw);
+        }
+        const int tt_lo = part == 1 ? my_gs + 2 * ngs : my_gs, tt_hi = part == 0 ? (gr < my_gs + 2 * ngs ? gr : my_gs + 2 * ngs) : gr;
+        for (int tt = tt_lo; tt < tt_hi; tt += ngs) {
+            const long long voff = vrow + (long long)(g_first + tt) * stride;
+            float2 d[RQ][2];
+#pragma unroll
+            for (int j = 0; j < RQ; j++)
+#pragma unroll
+                for (int k = 0; k < 2; k++) {
+                    const int t = m + k + j * NKc;
+                    float2 z;
+                    if (staged) {
+                        const int e = vmis[j] + tt * stride + 2 * mp + k;
+                        const unsigned char *row = sbuf + RQ * G.cp * 8 + j * G.vb;
+                        if constexpr (VDT == DT_CF32)
+                            z = t < L ? reinterpret_cast<const float2 *>(row)[e] : make_float2(0.f, 0.f);
+                        else
+                            z = t < L ? sc16_to_f32(reinterpret_cast<const uint32_t *>(row)[e]) : make_float2(0.f, 0.f);
+                    } else {
+                        z = t < L ? load_voltage<VDT>(P->V, voff + t) : make_float2(0.f, 0.f);
+                    }
+                    d[j][k] = cmul_conj(z, c[j][k]);
+                }
+            predecode_combine<RQ>(d, tw, NKc, reinterpret_cast<float4 *>(base + (size_t)(tt * RQ) * NKc + m));
+        }
+    }
+}
+
+// The common case of ring_produce_fn, kept lean: inputs staged in shared memory, code_len == N (no zero padding), and
+// at most one pair of inner indices per thread (gridDim.x >= 16).  Same arithmetic, same order.
+template <int RQ, int VDT>
+__device__ __noinline__ void ring_produce_lean_fn(const KParams *P, int sp, int part) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const RingGeo<RQ, VDT> G(P, smem);
+    constexpr int VESZ = RingGeo<RQ, VDT>::VESZ, NKc = RingGeo<RQ, VDT>::NK;
+    const int tid = threadIdx.x;
+    const int n_ipp = P->n_ipp, stride = P->stride;
+    const int kk = sp / n_ipp, pp = sp - kk * n_ipp;
+    const int g_first = kk * G.GR;
+    const int gr = (P->R - g_first) < G.GR ? (P->R - g_first) : G.GR;
+    const int npair = G.npair;
+    const int ngs = kFusedThreads / npair;
+    const int my_gs = tid / npair, mp = tid - my_gs * npair;
+    const unsigned char *sbuf = G.stage + (sp & 1) * G.buf;
+    mbar_wait(G.ctl + 48 + 8 * (uint32_t)(sp & 1), (uint32_t)(sp >> 1) & 1u);
+    if (my_gs >= ngs) return;
+    const int tt_lo = part == 1 ? my_gs + 2 * ngs : my_gs, tt_hi = part == 0 ? (gr < my_gs + 2 * ngs ? gr : my_gs + 2 * ngs) : gr;
+    if (tt_lo >= tt_hi) return;
+    // row j of the buffer starts at the 16-byte boundary at or below its first element: element index = mis_j + ...
+    const uintptr_t c0 = reinterpret_cast<uintptr_t>(P->C + (long long)pp * P->c_pitch + 2 * G.mp0);
+    const uintptr_t v0 = reinterpret_cast<uintptr_t>(P->V) +
+                         (uintptr_t)(((long long)pp * P->v_pitch + P->r0 + (long long)g_first * stride + 2 * G.mp0) * VESZ);
+    float2 c[RQ][2], tw[RQ - 1][2];
+    const unsigned char *vrow[RQ];
+#pragma unroll
+    for (int j = 0; j < RQ; j++) {
+        // N = RQ * 16384 samples of 8 (4) bytes apart: every row has the misalignment of row 0
+        const float2 *cj = reinterpret_cast<const float2 *>(sbuf + j * G.cp * 8) + (int)((c0 & 15) >> 3) + 2 * mp;
+        c[j][0] = cj[0];
+        c[j][1] = cj[1];
+        vrow[j] = sbuf + RQ * G.cp * 8 + j * G.vb + ((int)((v0 & 15) / VESZ) + 2 * mp + tt_lo * stride) * VESZ;
+    }
+#pragma unroll
+    for (int q = 1; q < RQ; q++) {
+        tw[q - 1][0] = G.tws[(q - 1) * 2 * G.npmax + 2 * mp];
+        tw[q - 1][1] = G.tws[(q - 1) * 2 * G.npmax + 2 * mp + 1];
+    }
+    float4 *out = reinterpret_cast<float4 *>(P->ring + ((size_t)(sp % P->ring_depth) * gridDim.x + (size_t)(tt_lo * RQ)) * (size_t)NKc +
+                                             2 * (G.mp0 + mp));
+    const int vstep = ngs * stride * VESZ;
+    const size_t ostep = (size_t)ngs * RQ * (NKc / 2);               // float4 elements between successive gates of a thread
+    for (int tt = tt_lo; tt < tt_hi; tt += ngs) {
+        float2 d[RQ][2];
+#pragma unroll
+        for (int j = 0; j < RQ; j++) {
+#pragma unroll
+            for (int k = 0; k < 2; k++) {
+                float2 z;
+                if constexpr (VDT == DT_CF32) z = reinterpret_cast<const float2 *>(vrow[j])[k];
+                else z = sc16_to_f32(reinterpret_cast<const uint32_t *>(vrow[j])[k]);
+                d[j][k] = cmul_conj(z, c[j][k]);
+            }
+            vrow[j] += vstep;
+        }
+        predecode_combine<RQ>(d, tw, NKc, out);
+        out += ostep;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // ST = true: the samples of IPP p that the CTA's gates touch (one contiguous run, overlapping windows
 // included once) are copied global -> shared by one cp.async.bulk per 32 KB while the CTA is still
 // transforming IPP p - 1; pass A then reads shared memory.  The copy starts at the 16-byte boundary at
@@ -225,9 +453,9 @@ __device__ __forceinline__ void bfly_dif_halves(float2 &r, float2 &i) {
 // a step that needs its own later work, so the grid cannot deadlock as long as all CTAs are resident.
 // The decoded windows never reach DRAM: the scratch round trip of the old split path (2 x 21 GB at cfg 4) is gone.
 template <int RA, int Q, int DT, bool ST, bool PFE = true, int RQ = 0, int VDT = DT_CF32>
-__global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P) {
+__global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_constant__ KParams P) {
     static_assert(!ST || Q == 1, "the staged variant holds one whole window run in shared memory");
-    static_assert(RQ == 0 || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && !PFE), "ring mode: 16384-point complex64 windows");
+    static_assert(RQ == 0 || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && PFE), "ring mode: 16384-point complex64 windows");
     constexpr int ESZ = DT == DT_CF32 ? 8 : 4;
     constexpr int NJ = 16 / RA;            // a' values per thread in pass A
     constexpr int G = 16 / RA;             // gates per CTA
@@ -320,6 +548,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             mbar_init(mbar, 1);
             *cnt = 0;
         }
+        if constexpr (RQ > 0) {
+            for (int i = 0; i < 16; i++) reinterpret_cast<int *>(smem + kFusedSmemBytes + kRingCtlOff)[i] = 0;
+            mbar_init(smem_u32(smem + kFusedSmemBytes + kRingCtlOff + 48), 1);
+            mbar_init(smem_u32(smem + kFusedSmemBytes + kRingCtlOff + 56), 1);
+        }
         fence_mbar_init();
         if constexpr (ST) {
             fence_proxy_async();
@@ -346,7 +579,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         if constexpr (DT == DT_SC16) {
             raw[i] = __ldg(b + (i >> 1) * 1024 + (i & 1) * 32);
         } else {
-            const uint2 v = __ldg(reinterpret_cast<const uint2 *>(b) + (i >> 1) * 1024 + (i & 1) * 32);
+            const uint2 *a = reinterpret_cast<const uint2 *>(b) + (i >> 1) * 1024 + (i & 1) * 32;
+            const uint2 v = RQ ? __ldcg(a) : __ldg(a);           // ring slots are rewritten during the launch: L2 only
             raw[2 * i] = v.x;
             raw[2 * i + 1] = v.y;
         }
@@ -359,48 +593,98 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
     }
 
-    // ---- ring mode: producer side and the two hand-over counters per slot
-    const int ringW = 16 * (int)gridDim.x;         // warp arrivals that complete a step
-    auto ring_wait = [&](int slot, int target) {   // slot < depth: ready counters, >= depth: done counters
+    // ---- ring mode: producer side and the two hand-over counters per slot.  Arrivals are counted per CTA in shared
+    // memory (by step & 3: the warps of a CTA are never more than a window or two apart) and the 16th warp of a step
+    // passes the CTA's arrival on to the global counter, so a step completes at gridDim.x arrivals; the first warp
+    // of a CTA that needs a step polls the global counter (one poller per CTA: every acquire load drops the SM's
+    // L1) and publishes what it saw in shared memory for the other fifteen.
+    const uint32_t ring_ctl = smem_u32(smem + kFusedSmemBytes + kRingCtlOff);   // +0 ready cnt[4], +16 done cnt[4], +32 seen[2], +40 lock[2], +48 stage mbarrier[2]
+    const bool r_staged = RQ > 0 && P.ring_stage != 0;
+    const bool r_lean = r_staged && P.L == P.N && gridDim.x >= 16 && (P.c_pitch & 1) == 0;   // see ring_produce_lean_fn
+    auto ring_arrive = [&](int which, int step) {       // which: 0 ready (after this warp's stores), 1 done (after its loads)
+        __syncwarp();
         if (lane == 0) {
-            const int *f = P.ring_flags + 32 * slot;
-            while (ld_acquire(f) < target) { }
+            const int old = atom_add_acq_rel_cta(ring_ctl + 16 * which + 4 * (int)(step & 3), 1);
+            if ((old & 15) == 15) {
+                red_release_add(P.ring_flags + 32 * (which * P.ring_depth + (int)(step % P.ring_depth)), 1);
+                if (which == 0 && r_staged && step + 2 < (int)T) {     // every warp has read buffer step & 1 for the last time
+                    fence_proxy_async();
+                    if constexpr (RQ > 0) ring_stage_issue_fn<RQ, VDT>(&P, step + 2);
+                }
+            }
+        }
+    };
+    auto ring_wait = [&](int which, int step) {         // until every CTA has arrived `which` for `step`
+        if (lane == 0) {
+            const uint32_t seen = ring_ctl + 32 + 4 * which, lock = ring_ctl + 40 + 4 * which;
+            const int *f = P.ring_flags + 32 * (which * P.ring_depth + (int)(step % P.ring_depth));
+            const int target = (int)(step / P.ring_depth + 1) * (int)gridDim.x;
+            int spins = 0;
+            while (ld_acquire_cta(seen) <= (int)step) {       // seen = number of leading steps known complete
+                if (atom_cas_acquire_cta(lock, 0, 1) == 0) {
+                    if (ld_acquire_cta(seen) <= (int)step) {
+                        // bounded: if the grid were not fully resident (it is launched cooperatively, so it is) the
+                        // wait would never end; after ~seconds give up, say so in the error word behind the
+                        // counters, and run on
+                        while (ld_acquire(f) < target) {
+                            __nanosleep(32);
+                            if (++spins > (1 << 22)) {
+                                atomicExch(P.ring_flags + 64 * P.ring_depth, 1);
+                                break;
+                            }
+                        }
+                        st_release_cta(seen, (int)step + 1);
+                    }
+                    st_release_cta(lock, 0);
+                } else {
+                    __nanosleep(64);                          // another warp of the CTA is polling: stay out of the issue slots
+                }
+            }
         }
         __syncwarp();
     };
-    auto ring_produce = [&](long long sp) {        // this CTA's slice of every window of step sp -> ring slot sp % depth
+    // part 0: the first two gates of every thread, part 1: the rest + the arrival (-1: everything)
+    auto ring_produce = [&](int sp, int part) {
         if constexpr (RQ > 0) {
-            constexpr int NKc = 1024 * RA;
-            const int kk = (int)(sp / P.n_ipp), pp = (int)(sp - (long long)kk * P.n_ipp);
-            const int GR = (int)gridDim.x / RQ, g_first = kk * GR;
-            const int gr = (P.R - g_first) < GR ? (P.R - g_first) : GR;
-            const int mp0 = (int)(((long long)blockIdx.x * (NKc / 2)) / gridDim.x);
-            const int mp1 = (int)((((long long)blockIdx.x + 1) * (NKc / 2)) / gridDim.x);
-            const int npair = mp1 - mp0, items = gr * npair;
-            const int slot = (int)(sp % P.ring_depth);
-            float2 *base = P.ring + (size_t)slot * gridDim.x * (size_t)NKc;
-            const float2 *Crow = P.C + (long long)pp * P.c_pitch;
-            for (int it = tid; it < items; it += kFusedThreads) {
-                const int tt = it / npair, m = 2 * (mp0 + it - tt * npair);
-                const long long voff = (long long)pp * P.v_pitch + P.r0 + (long long)(g_first + tt) * P.stride;
-                predecode_pair<RQ, VDT>(P.V, voff, Crow, P.L, NKc, P.twN, m,
-                                        reinterpret_cast<float4 *>(base + (size_t)(tt * RQ) * NKc + m));
-            }
-            __syncwarp();
-            if (lane == 0) red_release_add(P.ring_flags + 32 * slot, 1);
+            if (r_lean) ring_produce_lean_fn<RQ, VDT>(&P, sp, part);
+            else ring_produce_fn<RQ, VDT>(&P, sp, part);
+            if (part != 0) ring_arrive(0, sp);
         }
     };
+    auto pf_ring = [&](int step) {           // this thread's first sample of its window in the slot of `step`
+        return reinterpret_cast<const uint32_t *>(P.ring + ((size_t)(step % P.ring_depth) * gridDim.x + blockIdx.x) * (size_t)(1024 * RA) +
+                                                  64 * wa + lane);
+    };
     if constexpr (RQ > 0) {
-        for (long long sp = 0; sp < P.ring_ahead && sp < T; sp++) ring_produce(sp);
+        if (r_staged) {
+            ring_stage_prologue_fn<RQ, VDT>(&P, (int)T);
+            __syncthreads();
+        }
+        for (int sp = 0; sp < P.ring_ahead && sp < (int)T; sp++) ring_produce(sp, -1);
+        if constexpr (PF) {                                          // the first window
+            ring_wait(0, 0);
+            const uint32_t *b = pf_ring(0);
+            sfor<0, 32>([&](auto i_) { pf_load(b, i_); });
+        }
     }
 
     int left = (int)(i1 - i0);                     // items still to do, this one included
     int p_lo = p0;
+    // ring mode: a "tile" is a run of at most kRingFlushEvery pulses of one round -- two-level summation: fp32 sums of
+    // many |X|^2 lose low bits to the running total, so no more than that many are summed in registers before they go
+    // to S (the old scratch path flushed per batch of 10 as well)
+    const int r_nch = RQ ? (P.n_ipp + kRingFlushEvery - 1) / kRingFlushEvery : 1;
     for (int tile = tile0; left > 0; tile++, p_lo = 0) {                   // the tiles this CTA's run touches
-    const int p_hi = (P.n_ipp - p_lo) < left ? P.n_ipp : p_lo + left;
+    int kround = tile;
+    if constexpr (RQ > 0) {
+        kround = tile / r_nch;
+        p_lo = (tile - kround * r_nch) * kRingFlushEvery;
+    }
+    const int p_hi = RQ ? (P.n_ipp < p_lo + kRingFlushEvery ? P.n_ipp : p_lo + kRingFlushEvery)
+                        : ((P.n_ipp - p_lo) < left ? P.n_ipp : p_lo + left);
     left -= p_hi - p_lo;
     const bool more_tiles = left > 0;
-    const int gg = group_of(tile), q = resid_of(tile);
+    const int gg = group_of(kround), q = resid_of(tile);
     const int r = gg * G + g;
     const int r_ld = r < Rv ? r : Rv - 1;          // ragged last group: recompute a valid gate, never flush it
     const long long gate_off = (long long)P.r0 + (long long)r_ld * P.stride;
@@ -412,18 +696,20 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         const bool has_next = p + 1 < p_hi || more_tiles;
         const int p_next = p + 1 < p_hi ? p + 1 : 0;
         const int tile_next = p + 1 < p_hi ? tile : tile + 1;
-        long long rs = 0;                                            // ring mode: this step
+        int rs = 0;                                                  // ring mode: this step (the host keeps T below 2^20)
         if constexpr (RQ > 0) {
-            rs = (long long)tile * P.n_ipp + p;
-            const long long sp = rs + P.ring_ahead;
-            if (sp < T) {
-                // slot sp % depth last held step sp - depth: every warp of the grid has loaded it
-                if (sp >= P.ring_depth) ring_wait(P.ring_depth + (int)(sp % P.ring_depth), (int)(sp / P.ring_depth) * ringW);
-                ring_produce(sp);
-            }
-            ring_wait((int)(rs % P.ring_depth), (int)(rs / P.ring_depth + 1) * ringW);
-            if (r >= Rv) {                                           // a round with fewer virtual gates than CTAs
-                if (lane == 0) red_release_add(P.ring_flags + 32 * (P.ring_depth + (int)(rs % P.ring_depth)), 1);
+            rs = kround * P.n_ipp + p;
+            if (r >= Rv) {                                           // a round with fewer virtual gates than CTAs: produce only
+                const int sp = rs + P.ring_ahead;
+                if (sp < (int)T) {
+                    if (sp >= P.ring_depth) ring_wait(1, sp - P.ring_depth);
+                    ring_produce(sp, -1);
+                }
+                ring_arrive(1, rs);
+                if constexpr (PF) {                                  // (re-defines the prefetch registers, so that they
+                    const uint32_t *b = pf_ring(rs);                 // need not survive the producer above)
+                    sfor<0, 32>([&](auto i_) { pf_load(b, i_); });
+                }
                 continue;
             }
         }
@@ -439,13 +725,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         }
         float2 xr[16], xi[16];
         // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
-        if constexpr (RQ > 0) {                                      // decoded already: straight from the ring (L2, never L1)
-            const float2 *win = P.ring + ((size_t)(rs % P.ring_depth) * gridDim.x + blockIdx.x) * (size_t)(1024 * RA) + 64 * wa + lane;
+        if constexpr (RQ > 0) {                                      // decoded already (prefetched from the ring)
             sfor<0, RA>([&](auto th_) {
                 constexpr int th = decltype(th_)::value;
-                const float2 z0 = __ldcg(win + th * 1024), z1 = __ldcg(win + th * 1024 + 32);
-                xr[th] = make_float2(z0.x, z1.x);
-                xi[th] = make_float2(z0.y, z1.y);
+                xr[th] = make_float2(__uint_as_float(raw[4 * th]), __uint_as_float(raw[4 * th + 2]));
+                xi[th] = make_float2(__uint_as_float(raw[4 * th + 1]), __uint_as_float(raw[4 * th + 3]));
             });
         } else if (PF && bpsk) {
             if constexpr (PF) {
@@ -504,10 +788,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             constexpr int jj = decltype(jj_)::value;
             dft_packed<RA, jj * RA>(xr, xi);
         });
-        if constexpr (RQ > 0) {                                      // this warp's loads of the slot have all returned
-            __syncwarp();
-            if (lane == 0) red_release_add(P.ring_flags + 32 * (P.ring_depth + (int)(rs % P.ring_depth)), 1);
-        }
+        if constexpr (RQ > 0) ring_arrive(1, rs);                   // this warp's loads of the slot have all returned
         if constexpr (ST) {
             // this warp has consumed its samples of IPP p; the last of the 16 warps starts the copy of IPP p + 1
             __syncwarp();
@@ -557,6 +838,14 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
                 }
             });
         });
+        if constexpr (RQ > 0) {
+            // producer: the data registers are dead and the warp would only wait for the other warps' stores.  Slot sp % depth last held step sp - depth: every warp of the grid must have loaded it.
+            const int sp = rs + P.ring_ahead;
+            if (sp < (int)T && (wa & 1) == 0) {                   // even warps produce here, odd ones between B1 and B2:
+                if (sp >= P.ring_depth) ring_wait(1, sp - P.ring_depth);   // one half's stores drain while the other half computes
+                ring_produce(sp, -1);
+            }
+        }
         if constexpr (RA == 1) {
             __syncwarp();
         } else {
@@ -599,6 +888,13 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             });
         });
         __syncwarp();
+        if constexpr (RQ > 0) {                                  // producer, odd warps (data registers dead again)
+            const int sp = rs + P.ring_ahead;
+            if (sp < (int)T && (wa & 1) != 0) {
+                if (sp >= P.ring_depth) ring_wait(1, sp - P.ring_depth);
+                ring_produce(sp, -1);
+            }
+        }
         // ---- pass B2: lane = c; decimation-in-frequency radix-32 over b; .x = b, .y = b + 16
         {
             const float2 *src = reinterpret_cast<const float2 *>(region) + lane;
@@ -618,6 +914,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
         });
         dft_packed16_head(xr, xi);
         const uint32_t *pf_next = nullptr;
+        if constexpr (RQ > 0) {
+            if (has_next) ring_wait(0, rs + 1);                  // the next window is in the ring (it has been for a while)
+        }
         sfor<0, 8>([&](auto k_) {                                // last stage + |X|^2 + accumulate
             constexpr int k = decltype(k_)::value;
             constexpr int ia = brev<4>(k), ib = brev<4>(k + 8);
@@ -625,7 +924,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const KParams P
             if constexpr (PF) {                                  // eight registers just died: four words of the next window
                 // unconditional (the last window fetches its own samples again): every word is redefined in every
                 // window, so none of them stays live through passes A and B
-                if constexpr (k == 0) pf_next = has_next ? pf_base(tile_next, p_next) : pf_base(tile, p);
+                if constexpr (k == 0) {
+                    if constexpr (RQ > 0) pf_next = pf_ring(has_next ? rs + 1 : rs);
+                    else pf_next = has_next ? pf_base(tile_next, p_next) : pf_base(tile, p);
+                }
                 sfor<4 * k, 4 * k + 4>([&](auto i_) { pf_load(pf_next, i_); });
                 if constexpr (k == 7) {
                     if (bpsk) cw_pf = __ldg(P.Cbits + (long long)(has_next ? p_next : p) * 512 + wa * 32 + lane);

@@ -144,12 +144,47 @@ __global__ void pack_codes_kernel(const float2 *__restrict__ C, uint32_t *__rest
 //     X[((p R + r) Q + q) Nk + m] = (sum_j d_{p,r}[m + j Nk] W_Q^{jq}) W_N^{mq},   d = V conj(C),
 // so that step 2 (the fused kernel on R Q "virtual gates" of length Nk, identity code) reads each decoded
 // sample once instead of every (gate, q) CTA decoding the whole window again.
-// predecode_pair: the two adjacent inner indices m, m + 1 (m even) of one window -> one 16-byte store per residue
-// at out[q * Nk / 2] (out = the float4 that holds x_0[m], x_0[m + 1]).  voff = index of the window's first sample in V.
+// Outer radix-Q butterfly + twiddles of the two adjacent inner indices m, m + 1 (m even): d[j][k] = decoded sample
+// m + k + j Nk; tw[q - 1][k] = W_N^{(m + k) q}.  One 16-byte store per residue at out[q * Nk / 2] (out = the float4
+// that holds x_0[m], x_0[m + 1]).
+template <int Q>
+__device__ __forceinline__ void predecode_combine(const float2 (&d)[Q][2], const float2 (&tw)[Q - 1][2], int Nk, float4 *out) {
+    const long long qs = Nk / 2;                                     // float4 elements between residues
+    float2 x[Q][2];
+#pragma unroll
+    for (int k = 0; k < 2; k++) {
+        if constexpr (Q == 2) {
+            x[0][k] = cadd(d[0][k], d[1][k]);
+            x[1][k] = cmul(csub(d[0][k], d[1][k]), tw[0][k]);
+        } else {
+            static_assert(Q == 4, "outer radix must be 2 or 4");
+            const float2 e0 = cadd(d[0][k], d[2][k]), e1 = csub(d[0][k], d[2][k]);
+            const float2 o0 = cadd(d[1][k], d[3][k]), o1 = csub(d[1][k], d[3][k]);
+            x[0][k] = cadd(e0, o0);
+            x[1][k] = cmul(make_float2(e1.x + o1.y, e1.y - o1.x), tw[0][k]);        // e1 - i o1
+            x[2][k] = cmul(csub(e0, o0), tw[1][k]);
+            x[3][k] = cmul(make_float2(e1.x - o1.y, e1.y + o1.x), tw[2][k]);        // e1 + i o1
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < Q; q++) out[q * qs] = make_float4(x[q][0].x, x[q][0].y, x[q][1].x, x[q][1].y);
+}
+
+// W_N^{(m + k) q}, q = 1 .. Q - 1, k = 0, 1, from the full-circle table
+template <int Q>
+__device__ __forceinline__ void predecode_twiddles(const float2 *__restrict__ twN, int m, float2 (&tw)[Q - 1][2]) {
+#pragma unroll
+    for (int q = 1; q < Q; q++)
+#pragma unroll
+        for (int k = 0; k < 2; k++) tw[q - 1][k] = __ldg(twN + q * (m + k));
+}
+
+// predecode_pair: decode (zero-pad reading A6) + combine for one window; voff = index of the window's
+// first sample in V
 template <int Q, int DT>
 __device__ __forceinline__ void predecode_pair(const void *__restrict__ V, long long voff, const float2 *__restrict__ Crow,
                                                int L, int Nk, const float2 *__restrict__ twN, int m, float4 *out) {
-    float2 d[Q][2];
+    float2 d[Q][2], tw[Q - 1][2];
 #pragma unroll
     for (int j = 0; j < Q; j++)
 #pragma unroll
@@ -157,25 +192,8 @@ __device__ __forceinline__ void predecode_pair(const void *__restrict__ V, long 
             const int t = m + k + j * Nk;
             d[j][k] = t < L ? cmul_conj(load_voltage<DT>(V, voff + t), __ldg(Crow + t)) : make_float2(0.f, 0.f);
         }
-    const long long qs = Nk / 2;                                     // float4 elements between residues
-    float2 x[Q][2];
-#pragma unroll
-    for (int k = 0; k < 2; k++) {
-        if constexpr (Q == 2) {
-            x[0][k] = cadd(d[0][k], d[1][k]);
-            x[1][k] = cmul(csub(d[0][k], d[1][k]), __ldg(twN + m + k));
-        } else {
-            static_assert(Q == 4, "outer radix must be 2 or 4");
-            const float2 e0 = cadd(d[0][k], d[2][k]), e1 = csub(d[0][k], d[2][k]);
-            const float2 o0 = cadd(d[1][k], d[3][k]), o1 = csub(d[1][k], d[3][k]);
-            x[0][k] = cadd(e0, o0);
-            x[1][k] = cmul(make_float2(e1.x + o1.y, e1.y - o1.x), __ldg(twN + (m + k)));        // e1 - i o1
-            x[2][k] = cmul(csub(e0, o0), __ldg(twN + 2 * (m + k)));
-            x[3][k] = cmul(make_float2(e1.x - o1.y, e1.y + o1.x), __ldg(twN + 3 * (m + k)));    // e1 + i o1
-        }
-    }
-#pragma unroll
-    for (int q = 0; q < Q; q++) out[q * qs] = make_float4(x[q][0].x, x[q][0].y, x[q][1].x, x[q][1].y);
+    predecode_twiddles<Q>(twN, m, tw);
+    predecode_combine<Q>(d, tw, Nk, out);
 }
 
 // grid = (Nk / 512, R, IPPs of the batch); a thread takes two adjacent m

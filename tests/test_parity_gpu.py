@@ -193,13 +193,17 @@ def test_staged_and_direct_loads_agree(N, dtype, r0, stride):
 
 @pytest.mark.parametrize("N,dtype", [(32768, synth.CF32), (32768, synth.SC16), (65536, synth.CF32), (65536, synth.SC16)])
 def test_split_and_fully_fused_paths_agree_above_16384(N, dtype):
-    """N > 16384: the decode pre-pass + scratch path (default) and the fully fused path (every CTA decodes
-    its whole window) both meet the oracle; short code (zero-pad), odd stride, several scratch batches."""
+    """N > 16384: the decode pre-pass + scratch path (default), the ring path (one cooperative launch, decoded windows
+    handed over through L2) and the fully fused path (every CTA decodes its whole window) all meet the oracle;
+    short code (zero-pad), odd stride, several scratch batches."""
     w, V, C = random_case(N, N - 7, 3, 1, 5, 5, dtype)
     S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    S_ring, st1 = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, split=2)
     S_split, st = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, split=1, batch=2)      # 3 scratch batches
     S_fused, st0 = run_gpu(w, V, C, kernel=pl.KERNEL_FUSED, split=0)
-    assert gate_metric(S_split, S_ref).max() <= TOL and gate_metric(S_fused, S_ref).max() <= TOL
+    for S in (S_ring, S_split, S_fused):
+        assert gate_metric(S, S_ref).max() <= TOL
+    assert st1["kernel_launches"] == 1 + 1                        # ring kernel + un-permute
     assert st["kernel_launches"] == 3 * 2 + 1                     # (pre-pass + fused) per batch + un-permute
 
 
@@ -382,7 +386,7 @@ def test_split_option_toggled_on_one_handle_with_complex_code():
     v, c = to_dev(V), to_dev(C)
     out = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
     with pl.Integrator.for_workload(w, kernel=pl.KERNEL_FUSED) as it:
-        for split in (1, 0, 1, 0, 1):
+        for split in (1, 0, 2, 0, 2, 1, 0):
             pl.plspec_configure(it.h, pl.PLSPEC_OPT_SPLIT, split)
             it.accumulate(v, c, w.n_ipp)
             it.finalize(out)
@@ -506,3 +510,26 @@ def test_poisoned_guard_bands_around_inputs(N, L, dtype, stage):
         S = out.cpu().numpy()
         assert np.isfinite(S).all()
         assert gate_metric(S, S_ref).max() <= TOL
+
+
+# ---- ring mode (N > 16384): several lockstep rounds, ragged last round, every knob ---------------------------------
+@pytest.mark.parametrize("N,R,dtype,L,stride,depth,ahead", [
+    (65536, 41, synth.CF32, 65536, 4, 0, 0),        # 164 virtual gates: two rounds on 148 CTAs, the second ragged
+    (65536, 38, synth.SC16, 65536 - 9, 3, 2, 1),    # shortest ring; short code; sc16 producer
+    (32768, 80, synth.CF32, 32768, 1, 3, 2),        # outer radix 2: 74 gates per round
+    (32768, 5, synth.SC16, 20000, 7, 8, 5),         # fewer virtual gates than CTAs; deep ring
+    (65536, 75, synth.CF32, 65536, 2, 4, 3),        # three rounds
+])
+def test_ring_mode_rounds(N, R, dtype, L, stride, depth, ahead):
+    w, V, C = random_case(N, L, R, 2, stride, 3, dtype)
+    S_ref = oracle.spectra(V, C, N=w.N, n_ranges=w.n_ranges, r0=w.r0, stride=w.stride)
+    out = torch.empty((w.n_ranges, w.N), dtype=torch.float32, device="cuda")
+    v, c = to_dev(V), to_dev(C)
+    for stage in (1, 0):                                            # producer inputs through shared memory / from L2
+        with pl.Integrator.for_workload(w, split=2, ring_depth=depth, ring_ahead=ahead, stage=stage) as it:
+            for _ in range(3):                                      # the counters start over with every launch
+                it.accumulate(v[:1], c[:1], 1)
+                it.accumulate(v[1:], c[1:], w.n_ipp - 1)
+                it.finalize(out)
+                m = gate_metric(out.cpu().numpy(), S_ref)
+                assert m.max() <= TOL, f"stage {stage}: worst gate {int(m.argmax())}: {m.max():.3e}"
