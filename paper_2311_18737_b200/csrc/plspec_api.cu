@@ -255,7 +255,7 @@ __global__ void replicate_code_kernel(const float2 *__restrict__ code, float2 *_
 
 // Step 1 of a launch: bring the codes of n_ipp pulses into the form the kernels read (cp.C, cp.cbits).
 int prepare_codes(plspec_ctx *h, CodePrep &cp, const float2 *dC, int n_ipp, cudaStream_t stream) {
-    if (h->kind == 2 && h->ring_mode) {                  // the ring kernel reads the codes as given (row pitch 0 or L)
+    if (h->kind == 2 && (h->ring_mode || h->split)) {    // these paths read the codes as given (row pitch 0 or L)
         cp.C = dC; cp.packed = false; cp.epoch = 1;
         return PLSPEC_OK;
     }
@@ -309,7 +309,7 @@ int launch_gates(plspec_ctx *h, const CodePrep &cp, const void *dV, long long v_
     if (h->kind == 2 && h->ring_mode) return launch_ring(h, dV, cp.C, v_pitch, r0, n_ipp, g_lo, g_cnt, stream);
     if (h->kind == 2 && h->split) return launch_split(h, dV, cp.C, v_pitch, r0, n_ipp, g_lo, g_cnt, stream);
     const int n_groups = (g_cnt + h->gates_per_cta - 1) / h->gates_per_cta;
-    KParams P;
+    KParams P{};
     P.V = dV; P.C = cp.C; P.S = h->S + (size_t)g_lo * (size_t)h->N;
     P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
     P.v_pitch = v_pitch;
@@ -405,7 +405,7 @@ int launch_ring(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pit
     for (int p0 = 0; p0 < n_ipp; p0 += per_launch) {
         const int nb = n_ipp - p0 < per_launch ? n_ipp - p0 : per_launch;
         PL_CUDA(h, cudaMemsetAsync(h->ring_flags, 0, (size_t)2 * depth * 32 * sizeof(int), stream));
-        KParams P;
+        KParams P{};
         P.V = (const char *)dV + (size_t)p0 * (size_t)v_pitch * esz;
         P.C = dC + (size_t)p0 * (size_t)c_pitch;
         P.S = h->S + (size_t)g_lo * (size_t)h->N; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
@@ -470,24 +470,27 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
     const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
     for (int p0 = 0; p0 < n_ipp; p0 += (int)fit) {
         const int nb = n_ipp - p0 < (int)fit ? n_ipp - p0 : (int)fit;
-        KParams P;
+        KParams P{};
         P.V = (const char *)dV + (size_t)p0 * (size_t)v_pitch * esz;
-        P.C = dC + (size_t)p0 * h->L;
+        const int c_pitch = h->opt_shared_code ? 0 : h->L;            // the pre-pass reads the one code in place
+        P.C = dC + (size_t)p0 * (size_t)c_pitch;
         P.S = h->S + (size_t)g_lo * (size_t)h->N; P.twA = h->twA; P.twB = h->twB; P.twN = h->twN;
         P.Cbits = nullptr; P.not_bpsk = nullptr; P.epoch = 1;
         P.v_pitch = v_pitch;
         P.N = h->N; P.Nk = h->Nk; P.Q = h->Q; P.log2Nk = ilog2(h->Nk);
         P.L = h->L; P.R = g_cnt; P.r0 = r0 + g_lo * h->stride; P.stride = h->stride;
         P.n_groups = g_cnt; P.n_ipp = nb; P.n_chunks = 1; P.use_atomic = 0;
-        if (g_cnt > 65535) return PLSPEC_ERR_UNSUPPORTED;
-        const dim3 blocks((unsigned)(h->Nk / 512), (unsigned)g_cnt, (unsigned)nb);
+        P.ring = nullptr; P.ring_flags = nullptr; P.ring_depth = 0; P.ring_ahead = 0; P.c_pitch = c_pitch; P.ring_stage = 0;
+        constexpr int GB = 8;                                         // gates per thread of the pre-pass
+        if ((g_cnt + GB - 1) / GB > 65535) return PLSPEC_ERR_UNSUPPORTED;
+        const dim3 blocks((unsigned)(h->Nk / 512), (unsigned)((g_cnt + GB - 1) / GB), (unsigned)nb);
         const bool sc = h->dtype == PLSPEC_SC16;
         if (h->Q == 2) {
-            if (sc) predecode_kernel<2, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq);
-            else    predecode_kernel<2, DT_CF32><<<blocks, 256, 0, stream>>>(P, h->xq);
+            if (sc) predecode_kernel<2, DT_SC16, GB><<<blocks, 256, 0, stream>>>(P, h->xq);
+            else    predecode_kernel<2, DT_CF32, GB><<<blocks, 256, 0, stream>>>(P, h->xq);
         } else {
-            if (sc) predecode_kernel<4, DT_SC16><<<blocks, 256, 0, stream>>>(P, h->xq);
-            else    predecode_kernel<4, DT_CF32><<<blocks, 256, 0, stream>>>(P, h->xq);
+            if (sc) predecode_kernel<4, DT_SC16, GB><<<blocks, 256, 0, stream>>>(P, h->xq);
+            else    predecode_kernel<4, DT_CF32, GB><<<blocks, 256, 0, stream>>>(P, h->xq);
         }
         PL_CUDA(h, cudaGetLastError());
         h->stats.kernel_launches++;

@@ -196,14 +196,53 @@ __device__ __forceinline__ void predecode_pair(const void *__restrict__ V, long 
     predecode_combine<Q>(d, tw, Nk, out);
 }
 
-// grid = (Nk / 512, R, IPPs of the batch); a thread takes two adjacent m
-template <int Q, int DT>
+// grid = (Nk / 512, ceil(R / GB), IPPs of the batch); a thread takes two adjacent m of GB successive gates: the code
+// samples and the outer twiddles of its m are loaded once and stay in registers for all GB windows (they are the
+// same for every gate, and with stride << N the gates' echo samples overlap in L1 / L2), so that per decoded sample
+// one echo sample is loaded instead of echo + code + twiddles; two gates' loads are in flight at a time.
+// Code row of IPP p: P.C + p * P.c_pitch (c_pitch = 0: one code for every IPP, PLSPEC_OPT_SHARED_CODE).
+template <int Q, int DT, int GB>
 __global__ void __launch_bounds__(256) predecode_kernel(const KParams P, float2 *__restrict__ X) {
     const int m = 2 * (blockIdx.x * 256 + threadIdx.x);
-    const int r = blockIdx.y;
+    const int r0g = blockIdx.y * GB;
     const long long p = blockIdx.z;
-    predecode_pair<Q, DT>(P.V, p * P.v_pitch + P.r0 + (long long)r * P.stride, P.C + p * P.L, P.L, P.Nk, P.twN, m,
-                          reinterpret_cast<float4 *>(X + ((p * P.R + r) * Q) * P.Nk + m));
+    const float2 *Crow = P.C + p * P.c_pitch;
+    float2 c[Q][2], tw[Q - 1][2];
+#pragma unroll
+    for (int j = 0; j < Q; j++)
+#pragma unroll
+        for (int k = 0; k < 2; k++) {
+            const int t = m + k + j * P.Nk;
+            c[j][k] = t < P.L ? __ldg(Crow + t) : make_float2(0.f, 0.f);
+        }
+    predecode_twiddles<Q>(P.twN, m, tw);
+    const long long vrow = p * P.v_pitch + P.r0;
+    const int g_end = (P.R - r0g) < GB ? (P.R - r0g) : GB;
+    for (int g = 0; g < g_end; g += 2) {
+        const bool two = g + 1 < g_end;
+        float2 z[2][Q][2];
+#pragma unroll
+        for (int u = 0; u < 2; u++) {
+            const long long voff = vrow + (long long)(r0g + g + u) * P.stride;
+#pragma unroll
+            for (int j = 0; j < Q; j++)
+#pragma unroll
+                for (int k = 0; k < 2; k++) {
+                    const int t = m + k + j * P.Nk;
+                    z[u][j][k] = (t < P.L && (u == 0 || two)) ? load_voltage<DT>(P.V, voff + t) : make_float2(0.f, 0.f);
+                }
+        }
+#pragma unroll
+        for (int u = 0; u < 2; u++) {
+            if (u == 1 && !two) break;
+            float2 d[Q][2];
+#pragma unroll
+            for (int j = 0; j < Q; j++)
+#pragma unroll
+                for (int k = 0; k < 2; k++) d[j][k] = cmul_conj(z[u][j][k], c[j][k]);
+            predecode_combine<Q>(d, tw, P.Nk, reinterpret_cast<float4 *>(X + ((p * P.R + r0g + g + u) * Q) * P.Nk + m));
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------
