@@ -227,7 +227,7 @@ def ncu_traffic(name):
         return None, f"ncu_traffic.json unreadable: {type(e).__name__}"
 
 
-def products_timing(w, S_dev, flush, reps=7):
+def products_timing(w, S_dev, flush, reps=7, it=None, accumulate=None):
     """plspec_mean_spectrum (centred) and plspec_profile on the finished S: median of `reps` launches, L2 flushed
     before each, CUDA events on the current stream.  Both are one pass over S: algorithmic bytes 8 and 4 per bin,
     against the measured HBM copy peak (MEASURED_PEAKS.json, else the profiling guide's 6 550 GB/s fallback)."""
@@ -240,6 +240,15 @@ def products_timing(w, S_dev, flush, reps=7):
         peak, src = 6550.0, "fallback (B200_PROFILING.md)"
     P = torch.empty_like(S_dev)
     ki = torch.empty((2, R), dtype=torch.int32, device="cuda"); pf = torch.empty((3, R), dtype=torch.float32, device="cuda")
+    # These kernels are HBM-bound and last tens of microseconds.  After the write flush L2 is full of DIRTY lines whose
+    # write-back would be charged to the kernel that evicts them, so the write flush is followed by a read of a second
+    # buffer larger than L2: the kernel then starts from a cache of clean lines that hold none of its data.
+    clean = torch.zeros(flush.numel() // 4, dtype=torch.int32, device="cuda")
+
+    def flush_l2():
+        flush.fill_(3)
+        clean.sum()
+
     calls = {"mean_spectrum_centred": (8, lambda: pl.plspec_mean_spectrum(S_dev, P, R, N, w.n_ipp, True)),
              "profile": (4, lambda: pl.plspec_profile(S_dev, R, N, w.n_ipp, max(1, N // 256), 2, ki[0], pf[0], ki[1],
                                                       pf[1], pf[2]))}
@@ -247,7 +256,7 @@ def products_timing(w, S_dev, flush, reps=7):
     for name, (bpb, call) in calls.items():
         ts = []
         for _ in range(reps + 2):
-            flush.fill_(3)
+            flush_l2()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(); call(); e1.record()
             torch.cuda.synchronize()
@@ -255,6 +264,29 @@ def products_timing(w, S_dev, flush, reps=7):
         ms = float(np.median(ts[2:]))
         gbs = bpb * R * N / ms / 1e6
         out[name] = {"ms": ms, "bytes_per_bin": bpb, "GB/s": gbs, "frac": gbs / peak}
+    if it is not None:
+        # the write-out alone (plspec_finalize to device memory: 12 B per bin -- accumulators read and zeroed, S_out
+        # written) against the write-out with both products folded in (plspec_finalize_products: 16 B per bin, P_out
+        # besides; the stand-alone sequence finalize + mean + profile moves 24 B per bin); each after a fresh
+        # integration, L2 flushed, the blocking call between two events
+        k_min = max(1, N // 256)
+        fin = {"finalize": (12, lambda: it.finalize(S_dev)),
+               "finalize_products": (16, lambda: it.finalize_products(S_dev, w.n_ipp, P_out=P, centred=True, k_min=k_min, guard=2,
+                                                                      k_up=ki[0], p_up=pf[0], k_dn=ki[1], p_dn=pf[1],
+                                                                      noise=pf[2]))}
+        for name, (bpb, call) in fin.items():
+            ts = []
+            for _ in range(5):
+                accumulate()
+                torch.cuda.synchronize()
+                flush_l2()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); call(); e1.record()
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            ms = float(np.median(ts[1:]))
+            gbs = bpb * R * N / ms / 1e6
+            out[name] = {"ms": ms, "bytes_per_bin": bpb, "GB/s": gbs, "frac": gbs / peak}
     return out
 
 
@@ -475,7 +507,8 @@ def main():
     products = None
     if world == 1:
         try:
-            products = products_timing(w, S_dev, flush)
+            products = products_timing(w, S_dev, flush, it=it if mode == "replicas" else None,
+                                       accumulate=lambda: it.accumulate(V_dev, C_dev, n_ipp_local))
         except Exception as e:                                      # reported beside the metric: never fails the bench
             products = {"error": f"{type(e).__name__}: {e}"[:200]}
 

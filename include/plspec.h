@@ -175,6 +175,34 @@ int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, in
 int plspec_mean_spectrum(const float *S, float *P_out, int n_ranges, int N, int n_ipp, int centred, void *stream);
 
 /*
+ * EXTENSION (the row-wise products "fuse into finalize"): plspec_finalize to DEVICE memory
+ * with the products of plspec_mean_spectrum and / or plspec_profile computed in the same pass over the accumulators,
+ * while each gate's bins are being put into natural order -- S is read once; S_out and P_out are written once.
+ * Same definitions and the same results as the two stand-alone calls applied to S_out (line bins, powers and mean
+ * spectrum bit for bit; the noise floor to float64 summation order).
+ */
+typedef struct {
+    int    n_ipp;     /* pulses summed since the last finalize (>= 1): the divisor of Eq. 8's average  */
+    int    centred;   /* P_out: 0 = natural bin order, 1 = zero frequency at column N/2                             */
+    float *P_out;     /* [device] float[n_ranges][N], 16-byte aligned, or NULL: no mean spectrum                   */
+    int    k_min;     /* line search: 1 <= k_min < N/2 (see plspec_profile)                                         */
+    int    guard;     /* line search: >= 0                                                                          */
+    int   *k_up;      /* [device] int[n_ranges]   \                                                                 */
+    float *p_up;      /* [device] float[n_ranges]  |  all five, or all NULL: no line search                         */
+    int   *k_dn;      /* [device] int[n_ranges]    |                                                                */
+    float *p_dn;      /* [device] float[n_ranges]  |                                                                */
+    float *noise;     /* [device] float[n_ranges] /                                                                 */
+} plspec_products_t;
+/*
+ *   S_out  [device] float[n_ranges][N], 16-byte aligned: the un-normalised sum, as plspec_finalize writes it
+ *   prod   [host]   what else to compute; the struct is read during the call only
+ * Blocks until everything is written; zeroes the accumulators.  Errors: PLSPEC_ERR_INVALID_ARG (null handle / S_out /
+ * prod, host or misaligned pointers, P_out == S_out, some but not all line-search outputs, range errors),
+ * PLSPEC_ERR_CUDA.
+ */
+int plspec_finalize_products(plspec_handle h, float *S_out, const plspec_products_t *prod);
+
+/*
  * DIAGNOSTIC ("measured FMA peak to be reported beside" the derived one): the
  * FP32 multiply-add issue rate of the current device, the measured denominator of the path's ALU roofline
  * (5 N log2 N flop per decoded window).  Launches reps + 1 kernels of 4 x 512 threads per SM, each

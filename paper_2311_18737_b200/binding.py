@@ -42,7 +42,7 @@ LIB_PATH = os.path.join(_HERE, "libplspec.so")
 EXPORTED_SYMBOLS = (
     "plspec_create", "plspec_accumulate", "plspec_finalize", "plspec_reset", "plspec_destroy",
     "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_profile", "plspec_mean_spectrum",
-    "plspec_diag_fp32_peak",
+    "plspec_diag_fp32_peak", "plspec_finalize_products",
     "plspec_strerror",
     "plspec_version",
 )
@@ -57,6 +57,15 @@ class plspec_stats_t(ctypes.Structure):
         ("ipps_accumulated", ctypes.c_longlong),
         ("kernel_kind", ctypes.c_int),
         ("ipp_chunks_last", ctypes.c_int),
+    ]
+
+
+class plspec_products_t(ctypes.Structure):
+    _fields_ = [
+        ("n_ipp", ctypes.c_int), ("centred", ctypes.c_int), ("P_out", ctypes.c_void_p),
+        ("k_min", ctypes.c_int), ("guard", ctypes.c_int),
+        ("k_up", ctypes.c_void_p), ("p_up", ctypes.c_void_p), ("k_dn", ctypes.c_void_p), ("p_dn", ctypes.c_void_p),
+        ("noise", ctypes.c_void_p),
     ]
 
 
@@ -95,6 +104,7 @@ def lib() -> ctypes.CDLL:
         L.plspec_version.restype = ctypes.c_char_p
         L.plspec_profile.argtypes = [vp, ci, ci, ci, ci, ci, vp, vp, vp, vp, vp, vp]
         L.plspec_mean_spectrum.argtypes = [vp, vp, ci, ci, ci, ci, vp]
+        L.plspec_finalize_products.argtypes = [vp, vp, ctypes.POINTER(plspec_products_t)]
         L.plspec_diag_fp32_peak.argtypes = [ci, ci, ci, ctypes.POINTER(ctypes.c_double),
                                             ctypes.POINTER(ctypes.c_double), vp]
         for name in _INT_STATUS:
@@ -156,6 +166,14 @@ def plspec_accumulate(h, voltages, codes, n_ipp, stream=None) -> None:
 
 def plspec_finalize(h, S_out) -> None:
     _check(h, lib().plspec_finalize(h, _ptr(S_out)), "plspec_finalize")
+
+
+def plspec_finalize_products(h, S_out, n_ipp, P_out=None, centred=False, k_min=1, guard=0, k_up=None, p_up=None,
+                             k_dn=None, p_dn=None, noise=None) -> None:
+    prod = plspec_products_t(int(n_ipp), int(bool(centred)), _ptr(P_out) or None, int(k_min), int(guard),
+                             _ptr(k_up) or None, _ptr(p_up) or None, _ptr(k_dn) or None, _ptr(p_dn) or None,
+                             _ptr(noise) or None)
+    _check(h, lib().plspec_finalize_products(h, _ptr(S_out), ctypes.byref(prod)), "plspec_finalize_products")
 
 
 def plspec_profile(S, n_ranges, N, n_ipp, k_min, guard, k_up, p_up, k_dn, p_dn, noise, stream=None) -> None:
@@ -243,6 +261,10 @@ class Integrator:
 
     def finalize(self, S_out):
         plspec_finalize(self.h, S_out)
+        return S_out
+
+    def finalize_products(self, S_out, n_ipp, **products):
+        plspec_finalize_products(self.h, S_out, n_ipp, **products)
         return S_out
 
     def reset(self):

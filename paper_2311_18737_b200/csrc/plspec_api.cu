@@ -95,6 +95,7 @@ struct plspec_ctx {
     // device state
     float  *S = nullptr;             // [R][Q][Nk]
     float  *S_tmp = nullptr;         // un-permute target when S_out is a host pointer
+    void   *prod_work = nullptr;     // plspec_finalize_products: ProductsWork[R]
     float2 *twA = nullptr, *twB = nullptr, *twN = nullptr;
     CodePrep cp;                     // codes of the launch in flight
     int *not_bpsk = nullptr;         // device flags written by pack_codes_kernel: [0] cp, [2] tail.cp; [1]: never
@@ -703,6 +704,7 @@ void free_ctx(plspec_ctx *h) {
     }
     if (h->S) cudaFree(h->S);
     if (h->S_tmp) cudaFree(h->S_tmp);
+    if (h->prod_work) cudaFree(h->prod_work);
     if (h->twA) cudaFree(h->twA);
     if (h->twB) cudaFree(h->twB);
     if (h->twN) cudaFree(h->twN);
@@ -926,6 +928,65 @@ int plspec_finalize(plspec_handle h, float *S_out) {
             return PLSPEC_ERR_CUDA;
         }
     }
+    return PLSPEC_OK;
+}
+
+int plspec_finalize_products(plspec_handle h, float *S_out, const plspec_products_t *prod) {
+    if (!h || !S_out || !prod) return PLSPEC_ERR_INVALID_ARG;
+    const bool want_prof = prod->k_up || prod->p_up || prod->k_dn || prod->p_dn || prod->noise;
+    if (want_prof && !(prod->k_up && prod->p_up && prod->k_dn && prod->p_dn && prod->noise)) return PLSPEC_ERR_INVALID_ARG;
+    if (prod->n_ipp < 1 || (prod->centred != 0 && prod->centred != 1)) return PLSPEC_ERR_INVALID_ARG;
+    if (want_prof && (prod->k_min < 1 || prod->k_min >= h->N / 2 || prod->guard < 0)) return PLSPEC_ERR_INVALID_ARG;
+    if (prod->P_out == S_out) return PLSPEC_ERR_INVALID_ARG;
+    const void *ptrs[] = {S_out, prod->P_out, prod->k_up, prod->p_up, prod->k_dn, prod->p_dn, prod->noise};
+    for (const void *p : ptrs) {                         // device (or managed) memory only
+        if (!p) continue;
+        int dev = 0, rc = pointer_is_device(h, p, &dev);
+        if (rc != PLSPEC_OK) return rc;
+        if (!dev) return PLSPEC_ERR_INVALID_ARG;
+    }
+    if (((uintptr_t)S_out & 15) || ((uintptr_t)prod->P_out & 15)) return PLSPEC_ERR_INVALID_ARG;
+    cudaStream_t st = h->last_stream;
+    int rc = flush_tail(h, st);
+    if (rc != PLSPEC_OK) return rc;
+    const size_t total = (size_t)h->R * (size_t)h->N;
+    if (h->Q > 1 || h->kind == 2) {
+        // one pass over S_dev: transposition to natural order, zeroing, mean spectrum and line search
+        const int RAe = h->kind == 2 ? h->RA : 1, NC = h->kind == 2 ? 1024 : h->Nk, M = h->Q * RAe;
+        const int TC = 4096 / M < NC ? 4096 / M : NC;
+        ProductsWork *work = nullptr;
+        if (want_prof) {
+            if (!h->prod_work && cudaMalloc((void **)&h->prod_work, sizeof(ProductsWork) * (size_t)h->R) != cudaSuccess) {
+                (void)cudaGetLastError();
+                return PLSPEC_ERR_ALLOC;
+            }
+            work = static_cast<ProductsWork *>(h->prod_work);
+            PL_CUDA(h, cudaMemsetAsync(work, 0, sizeof(ProductsWork) * (size_t)h->R, st));
+        }
+        finalize_products_kernel<<<dim3((unsigned)h->R, (unsigned)(NC / TC)), 256, (size_t)TC * (M + 1) * sizeof(float), st>>>(
+            h->S, S_out, ilog2(h->Q), ilog2(RAe), NC, TC, prod->P_out, prod->centred, prod->n_ipp, prod->k_min, work);
+        PL_CUDA(h, cudaGetLastError());
+        h->stats.kernel_launches++;
+        if (want_prof) {
+            products_tail_kernel<<<(unsigned)((h->R + 3) / 4), 128, 0, st>>>(S_out, work, h->R, h->N, prod->n_ipp, prod->k_min,
+                                                                            prod->guard, prod->k_up, prod->p_up, prod->k_dn,
+                                                                            prod->p_dn, prod->noise);
+            PL_CUDA(h, cudaGetLastError());
+            h->stats.kernel_launches++;
+        }
+    } else {
+        // generic kernel, N <= 16384: S_dev is in natural order already; the stand-alone product kernels follow the copy
+        PL_CUDA(h, cudaMemcpyAsync(S_out, h->S, total * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        PL_CUDA(h, cudaMemsetAsync(h->S, 0, total * sizeof(float), st));
+        if (prod->P_out && (rc = plspec_mean_spectrum(S_out, prod->P_out, h->R, h->N, prod->n_ipp, prod->centred, st)) != PLSPEC_OK)
+            return rc;
+        if (want_prof && (rc = plspec_profile(S_out, h->R, h->N, prod->n_ipp, prod->k_min, prod->guard, prod->k_up, prod->p_up,
+                                              prod->k_dn, prod->p_dn, prod->noise, st)) != PLSPEC_OK)
+            return rc;
+        h->stats.kernel_launches += (prod->P_out ? 1 : 0) + (want_prof ? 1 : 0);
+    }
+    PL_CUDA(h, cudaStreamSynchronize(st));
+    h->have_work = false;
     return PLSPEC_OK;
 }
 

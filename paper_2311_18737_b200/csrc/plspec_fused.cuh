@@ -999,4 +999,122 @@ __global__ void __launch_bounds__(256) finalize_kernel(float *__restrict__ Sdev,
     }
 }
 
+// Finalize with the post-integration products folded into the write-out ("a row-wise reduction
+// that fuses into finalize"): finalize_kernel's transposition, same grid (gate, column tile), and while a tile's bins
+// pass through the CTA in natural order they are also (optionally) divided by n_ipp and written to P_out
+// (Eq. 8, centred or not) and fed to the arg maxima / float64 sum of plspec_profile (profile_kernel has
+// the definitions).  S is read once and S_out, P_out written once: no extra pass.  The CTAs of a gate meet in a
+// 32-byte workspace per gate (zeroed by the caller): the arg maxima as 64-bit keys (value bits << 32 | ~bin: S >= 0,
+// so the float's bit pattern orders like its value, and the lowest bin wins a tie) through atomicMax, the sum through a
+// float64 atomicAdd; products_tail_kernel then takes the bins near the lines out of the sum again and writes the five
+// per-gate numbers.
+struct ProductsWork { unsigned long long up, dn; double sum; unsigned long long pad; };
+
+__global__ void __launch_bounds__(256) finalize_products_kernel(float *__restrict__ Sdev, float *__restrict__ Sout, int log2Q,
+                                                                int log2RAe, int NC, int TC, float *__restrict__ Pout, int centred,
+                                                                int n_ipp, int k_min, ProductsWork *__restrict__ work) {
+    extern __shared__ float tile[];
+    __shared__ unsigned long long sb[2][8];
+    __shared__ double ssum[8];
+    const int log2M = log2Q + log2RAe, M = 1 << log2M, Q = 1 << log2Q, RAe = 1 << log2RAe;
+    const long long gate = blockIdx.x;
+    const int c0 = blockIdx.y * TC;
+    const int N = M * NC, n = M * TC;
+    float *X = Sdev + gate * (long long)N;
+    float *Yrow = Sout + gate * (long long)N;
+    float *Prow = Pout ? Pout + gate * (long long)N : nullptr;
+    int log2TC = 0;
+    while ((1 << log2TC) < TC) log2TC++;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lo = k_min, hi = N - k_min, mid = N / 2, half = centred ? N / 2 : 0;
+    const float dn_ipp = (float)n_ipp;
+    auto src_of = [&](int i) { return X + (long long)(i >> log2TC) * NC + c0 + (i & (TC - 1)); };
+    for (int i0 = tid; i0 < n; i0 += 8 * 256) {                         // eight independent loads in flight per thread
+        float v[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            const int i = i0 + u * 256;
+            v[u] = i < n ? __ldcs(src_of(i)) : 0.0f;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            const int i = i0 + u * 256;
+            const int j = i >> log2TC, c = i & (TC - 1);
+            const int q = j >> log2RAe, f_hi = j & (RAe - 1);
+            if (i < n) tile[c * (M + 1) + f_hi * Q + q] = v[u];
+        }
+    }
+    __syncthreads();
+    unsigned long long up = 0, dn = 0;                                 // key 0 = "no bin": below every real key
+    // a thread meets at most 16 bins: their sum in float32 (sequential: <= 15 roundings of 2^-24 relative, against the
+    // 1e-6 the noise floor is good to), the CTA's and the gate's sums in float64 -- float64 adds are scarce on this part
+    float facc = 0.f;
+    const int f0 = c0 * M;                                              // first natural bin of this tile
+    for (int i = tid; i < n; i += 256) {
+        const float x = tile[i + (i >> log2M)];
+        const int f = f0 + i;
+        Yrow[f] = x;
+        *src_of(i) = 0.0f;
+        if (Prow) Prow[(f + half) & (N - 1)] = __fdiv_rn(x, dn_ipp);
+        if (work && f >= lo && f <= hi && f != mid) {
+            const unsigned long long key = ((unsigned long long)__float_as_uint(x) << 32) | (unsigned)(~f);
+            if (f < mid) up = key > up ? key : up; else dn = key > dn ? key : dn;
+            facc += x;
+        }
+    }
+    if (!work) return;
+    double acc = (double)facc;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        const unsigned long long u = __shfl_xor_sync(0xffffffffu, up, o), d = __shfl_xor_sync(0xffffffffu, dn, o);
+        up = u > up ? u : up; dn = d > dn ? d : dn;
+        acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    }
+    if (lane == 0) { sb[0][warp] = up; sb[1][warp] = dn; ssum[warp] = acc; }
+    __syncthreads();
+    if (tid == 0) {
+        for (int w = 1; w < 8; w++) {
+            up = sb[0][w] > up ? sb[0][w] : up; dn = sb[1][w] > dn ? sb[1][w] : dn;
+            acc += ssum[w];
+        }
+        if (up) atomicMax(&work[gate].up, up);
+        if (dn) atomicMax(&work[gate].dn, dn);
+        atomicAdd(&work[gate].sum, acc);
+    }
+}
+
+// one warp per gate: the five numbers of plspec_profile from the workspace and the finished row of S_out
+__global__ void __launch_bounds__(128) products_tail_kernel(const float *__restrict__ Sout, const ProductsWork *__restrict__ work,
+                                                            int R, int N, int n_ipp, int k_min, int guard, int *__restrict__ k_up,
+                                                            float *__restrict__ p_up, int *__restrict__ k_dn,
+                                                            float *__restrict__ p_dn, float *__restrict__ noise) {
+    const int gate = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (gate >= R) return;
+    const float *row = Sout + (long long)gate * N;
+    const int lo = k_min, hi = N - k_min, mid = N / 2;
+    const ProductsWork w = work[gate];
+    const int ku = (int)~(unsigned)(w.up & 0xffffffffu), kd = (int)~(unsigned)(w.dn & 0xffffffffu);
+    const int g = guard < N ? guard : N, wlen = 2 * g + 1;
+    double ex = 0.0;
+    int nex = 0;
+    for (int j = lane; j < 2 * wlen; j += 32) {                         // the bins within `guard` of either line, each once
+        const bool second = j >= wlen;
+        const int f = (second ? kd : ku) - g + (second ? j - wlen : j);
+        const int du = f > ku ? f - ku : ku - f;
+        if (f >= lo && f <= hi && f != mid && !(second && du <= g)) { ex += (double)row[f]; nex++; }
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        ex += __shfl_xor_sync(0xffffffffu, ex, o);
+        nex += __shfl_xor_sync(0xffffffffu, nex, o);
+    }
+    if (lane == 0) {
+        k_up[gate] = ku; k_dn[gate] = kd;
+        p_up[gate] = __uint_as_float((unsigned)(w.up >> 32)) / (float)n_ipp;
+        p_dn[gate] = __uint_as_float((unsigned)(w.dn >> 32)) / (float)n_ipp;
+        const int cnt = (hi - lo) - nex;                               // hi - lo + 1 searched bins less N/2
+        noise[gate] = cnt > 0 ? (float)((w.sum - ex) / (double)cnt / (double)n_ipp) : 0.f;
+    }
+}
+
 }  // namespace plspec

@@ -286,6 +286,10 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
             const int i = i0 + u * 256;
             v[u] = i < nv ? __ldg(row4 + i) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
+        // interior vectors: the four bins summed in float32, the eight vectors of a batch pairwise in float32 (32 bins:
+        // five roundings of 2^-24 relative, against the 1e-6 the noise floor is good to), everything above in float64
+        // -- float64 adds are scarce on this part
+        float fs[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int u = 0; u < 8; u++) {
             const int i = i0 + u * 256;
@@ -297,11 +301,12 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
                 if (v[u].z > c.v) c = {v[u].z, f0 + 2};
                 if (v[u].w > c.v) c = {v[u].w, f0 + 3};
                 if (f0 < mid) up = better(up, c); else dn = better(dn, c);
-                acc += ((double)v[u].x + (double)v[u].y) + ((double)v[u].z + (double)v[u].w);
+                fs[u] = (v[u].x + v[u].y) + (v[u].z + v[u].w);
             } else {
                 take(v[u].x, f0); take(v[u].y, f0 + 1); take(v[u].z, f0 + 2); take(v[u].w, f0 + 3);
             }
         }
+        acc += (double)(((fs[0] + fs[1]) + (fs[2] + fs[3])) + ((fs[4] + fs[5]) + (fs[6] + fs[7])));
     }
 #pragma unroll
     for (int o = 16; o; o >>= 1) {

@@ -160,3 +160,70 @@ def test_products_on_a_user_stream_and_misaligned_profile_input():
     ki = torch.zeros(3, dtype=torch.int32, device="cuda"); pf = torch.zeros(3, dtype=torch.float32, device="cuda")
     with pytest.raises(pl.PlspecError):
         pl.plspec_profile(buf[1:], 3, 64, 1, 2, 0, ki, pf, ki, pf, pf)
+
+
+# ---- the products folded into the write-out: plspec_finalize_products ------------------------------------------------
+@pytest.mark.parametrize("N,R,dtype,kernel", [(1024, 19, synth.CF32, pl.KERNEL_FUSED), (4096, 11, synth.SC16, pl.KERNEL_FUSED),
+                                              (16384, 5, synth.SC16, pl.KERNEL_FUSED), (65536, 3, synth.CF32, pl.KERNEL_FUSED),
+                                              (32768, 3, synth.SC16, pl.KERNEL_FUSED), (256, 9, synth.CF32, pl.KERNEL_GENERIC),
+                                              (2048, 7, synth.CF32, pl.KERNEL_GENERIC)])
+def test_finalize_products_equals_finalize_then_products(N, R, dtype, kernel):
+    """One pass: S_out must be the spectrum the oracle computes, and the mean spectrum / line search must be exactly
+    what their oracles give ON THAT S_out (bins, powers, mean bit for bit; noise floor to summation order)."""
+    rng = np.random.default_rng(N + R)
+    P, L = 4, N
+    M = 2 + (R - 1) * 3 + L
+    C = (2.0 * rng.integers(0, 2, size=(P, L)) - 1.0).astype(np.complex64)
+    if dtype == synth.CF32:
+        V = (rng.standard_normal((P, M)) + 1j * rng.standard_normal((P, M))).astype(np.complex64)
+    else:
+        V = rng.integers(-2000, 2000, size=(P, M, 2)).astype(np.int16)
+    S_ref = oracle.spectra(V, C, N=N, n_ranges=R, r0=2, stride=3)
+    v, c = torch.from_numpy(V).cuda(), torch.from_numpy(C).cuda()
+    k_min, guard = max(1, N // 256), 2
+    with pl.Integrator(N, L, R, 2, 3, M, dtype, kernel=kernel) as it:
+        for centred, with_mean, with_prof in ((True, True, True), (False, True, False), (False, False, True)):
+            S = torch.full((R, N), -1.0, dtype=torch.float32, device="cuda")
+            Pm = torch.full((R, N), -1.0, dtype=torch.float32, device="cuda")
+            ki = torch.full((2, R), -7, dtype=torch.int32, device="cuda")
+            pf = torch.full((3, R), -1.0, dtype=torch.float32, device="cuda")
+            it.accumulate(v, c, P)
+            kw = {}
+            if with_mean:
+                kw.update(P_out=Pm, centred=centred)
+            if with_prof:
+                kw.update(k_min=k_min, guard=guard, k_up=ki[0], p_up=pf[0], k_dn=ki[1], p_dn=pf[1], noise=pf[2])
+            it.finalize_products(S, P, **kw)
+            S_h = S.cpu().numpy()
+            m = np.abs(S_h.astype(np.float64) - S_ref).max(axis=1) / S_ref.mean(axis=1)
+            assert m.max() <= 1e-4
+            if with_mean:
+                assert np.array_equal(Pm.cpu().numpy(), oracle.mean_spectrum(S_h, P, centred))
+            else:
+                assert float(Pm.min()) == -1.0 and float(Pm.max()) == -1.0
+            if with_prof:
+                ref = oracle.profile(S_h, P, k_min, guard)
+                assert np.array_equal(ki[0].cpu().numpy(), ref[0]) and np.array_equal(ki[1].cpu().numpy(), ref[2])
+                assert np.array_equal(pf[0].cpu().numpy(), ref[1]) and np.array_equal(pf[1].cpu().numpy(), ref[3])
+                assert np.allclose(pf[2].cpu().numpy(), ref[4], rtol=1e-6, atol=0)
+            it.finalize(S)                                        # the accumulators were zeroed by the fused call
+            assert float(S.abs().max()) == 0.0
+
+
+def test_finalize_products_argument_errors():
+    with pl.Integrator(1024, 1024, 4) as it:
+        S = torch.zeros((4, 1024), dtype=torch.float32, device="cuda")
+        ki = torch.zeros((2, 4), dtype=torch.int32, device="cuda")
+        pf = torch.zeros((3, 4), dtype=torch.float32, device="cuda")
+        bad = [dict(n_ipp=0), dict(n_ipp=1, P_out=S),                                        # aliasing
+               dict(n_ipp=1, k_up=ki[0]),                                                    # some but not all outputs
+               dict(n_ipp=1, k_min=0, k_up=ki[0], p_up=pf[0], k_dn=ki[1], p_dn=pf[1], noise=pf[2]),
+               dict(n_ipp=1, k_min=512, k_up=ki[0], p_up=pf[0], k_dn=ki[1], p_dn=pf[1], noise=pf[2]),
+               dict(n_ipp=1, P_out=np.zeros((4, 1024), np.float32))]                          # host pointer
+        for kw in bad:
+            n = kw.pop("n_ipp")
+            with pytest.raises(pl.PlspecError) as e:
+                it.finalize_products(S, n, **kw)
+            assert e.value.status == pl.PLSPEC_ERR_INVALID_ARG
+        with pytest.raises(pl.PlspecError):
+            it.finalize_products(np.zeros((4, 1024), np.float32), 1)                          # host S_out
