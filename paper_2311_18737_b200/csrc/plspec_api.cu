@@ -85,8 +85,6 @@ struct plspec_ctx {
     const void *kfunc_split = nullptr;   // fused_kernel<16, 1, CF32, false>
     float2 *xq = nullptr;                // [batch][R][Q][Nk]
     long long xq_ipps = 0;               // IPPs the scratch holds
-    uint32_t *zero_bits = nullptr;       // identity "code" for step 2: all signs +
-    long long zero_bits_words = 0;
     bool staged = false;             // fused kernel reads voltages through the shared-memory stage
     int block = 0;
     size_t smem = 0;
@@ -98,8 +96,7 @@ struct plspec_ctx {
     void   *prod_work = nullptr;     // plspec_finalize_products: ProductsWork[R]
     float2 *twA = nullptr, *twB = nullptr, *twN = nullptr;
     CodePrep cp;                     // codes of the launch in flight
-    int *not_bpsk = nullptr;         // device flags written by pack_codes_kernel: [0] cp, [2] tail.cp; [1]: never
-                                     // written, always 0
+    int *not_bpsk = nullptr;         // device flags written by pack_codes_kernel: [0] cp, [2] tail.cp
     int epoch = 0;                   // number of the last code pre-pass
     // host pipeline
     cudaStream_t copy_stream = nullptr;
@@ -201,7 +198,8 @@ int select_kernel(plspec_ctx *h) {
             if (occ_ring < 1) return PLSPEC_ERR_UNSUPPORTED;
         }
         if (h->split) {
-            h->kfunc_split = fused_lookup(16, 1, DT_CF32, false, true);   // scratch windows are whole: Nk samples each
+            // scratch windows are whole (Nk samples each) and decoded already: prefetching variant, identity code
+            h->kfunc_split = (const void *)fused_kernel<16, 1, DT_CF32, false, true, 0, DT_CF32, true>;
             PL_CUDA(h, cudaFuncSetAttribute(h->kfunc_split, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageOff));
         }
     } else {
@@ -457,17 +455,6 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
     long long fit = h->xq_ipps * per_ipp_full / per_ipp;               // IPPs of g_cnt gates the scratch holds
     if (h->opt_batch > 0 && fit > h->opt_batch) fit = h->opt_batch;
     if (fit > 65535) fit = 65535;
-    if (fit * 512 > h->zero_bits_words) {
-        if (h->zero_bits) cudaFree(h->zero_bits);
-        h->zero_bits = nullptr;
-        h->zero_bits_words = fit * 512;
-        if (cudaMalloc((void **)&h->zero_bits, sizeof(uint32_t) * (size_t)h->zero_bits_words) != cudaSuccess) {
-            (void)cudaGetLastError();
-            h->zero_bits_words = 0;
-            return PLSPEC_ERR_ALLOC;
-        }
-        PL_CUDA(h, cudaMemsetAsync(h->zero_bits, 0, sizeof(uint32_t) * (size_t)h->zero_bits_words, stream));
-    }
     const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
     for (int p0 = 0; p0 < n_ipp; p0 += (int)fit) {
         const int nb = n_ipp - p0 < (int)fit ? n_ipp - p0 : (int)fit;
@@ -498,9 +485,7 @@ int launch_split(plspec_ctx *h, const void *dV, const float2 *dC, long long v_pi
         // step 2: g_cnt * Q virtual gates, window = Nk contiguous decoded samples, identity code
         KParams F = P;
         F.V = h->xq; F.C = dC;
-        // sign-flip decode, no flips.  The flag word is the handle's permanent zero, not one pack_codes_kernel
-        // writes: an earlier launch of the unsplit path on this handle may have left any epoch in those.
-        F.Cbits = h->zero_bits; F.not_bpsk = h->not_bpsk + 1; F.epoch = 1;
+        F.Cbits = nullptr; F.not_bpsk = nullptr; F.epoch = 1;         // the kernel variant takes the windows as decoded
         F.v_pitch = per_ipp;
         F.N = h->Nk; F.Q = 1; F.L = h->Nk;
         F.R = g_cnt * h->Q; F.r0 = 0; F.stride = h->Nk;
@@ -722,7 +707,6 @@ void free_ctx(plspec_ctx *h) {
     if (h->xq) cudaFree(h->xq);
     if (h->ring) cudaFree(h->ring);
     if (h->ring_flags) cudaFree(h->ring_flags);
-    if (h->zero_bits) cudaFree(h->zero_bits);
     if (h->not_bpsk) cudaFree(h->not_bpsk);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     if (h->work_done) cudaEventDestroy(h->work_done);

@@ -452,10 +452,13 @@ __device__ __noinline__ void ring_produce_lean_fn(const KParams *P, int sp, int 
 // slot i serves steps i, i + depth, ... and step s completes at (s / depth + 1) * 16 gridDim.x.  A CTA never waits for
 // a step that needs its own later work, so the grid cannot deadlock as long as all CTAs are resident.
 // The decoded windows never reach DRAM: the scratch round trip of the old split path (2 x 21 GB at cfg 4) is gone.
-template <int RA, int Q, int DT, bool ST, bool PFE = true, int RQ = 0, int VDT = DT_CF32>
+// IDC = true: identity code -- the windows are decoded already (step 2 of the scratch path for N > 16384): pass A
+// takes the prefetched complex64 words as they are (no code words, no sign flips).
+template <int RA, int Q, int DT, bool ST, bool PFE = true, int RQ = 0, int VDT = DT_CF32, bool IDC = false>
 __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_constant__ KParams P) {
     static_assert(!ST || Q == 1, "the staged variant holds one whole window run in shared memory");
     static_assert(RQ == 0 || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && PFE), "ring mode: 16384-point complex64 windows");
+    static_assert(!IDC || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && PFE && RQ == 0), "identity code: prefetching complex64 variant");
     constexpr int ESZ = DT == DT_CF32 ? 8 : 4;
     constexpr int NJ = 16 / RA;            // a' values per thread in pass A
     constexpr int G = 16 / RA;             // gates per CTA
@@ -508,7 +511,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     tmem_wait_st();
 
     pdl_wait();   // everything above (TMEM, twiddles) may overlap the code pre-pass / decode pre-pass before us
-    const bool bpsk = P.Cbits != nullptr && __ldg(P.not_bpsk) != P.epoch;   // warp-uniform
+    const bool bpsk = IDC || (P.Cbits != nullptr && __ldg(P.not_bpsk) != P.epoch);   // warp-uniform
 
     unsigned char *const region = smem + warp * kRegionBytes;              // this warp's pass-B region
     unsigned char *const gate_regions = smem + (g * RA) * kRegionBytes;    // regions of this gate (pass A target)
@@ -589,7 +592,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
         if (bpsk) {
             const uint32_t *b = pf_base(tile0, p0);
             sfor<0, 32>([&](auto i_) { pf_load(b, i_); });
-            cw_pf = __ldg(P.Cbits + (long long)p0 * 512 + wa * 32 + lane);
+            if constexpr (!IDC) cw_pf = __ldg(P.Cbits + (long long)p0 * 512 + wa * 32 + lane);
         }
     }
 
@@ -725,7 +728,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
         }
         float2 xr[16], xi[16];
         // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
-        if constexpr (RQ > 0) {                                      // decoded already (prefetched from the ring)
+        if constexpr (RQ > 0 || IDC) {                               // decoded already (prefetched from the ring / the scratch)
             sfor<0, RA>([&](auto th_) {
                 constexpr int th = decltype(th_)::value;
                 xr[th] = make_float2(__uint_as_float(raw[4 * th]), __uint_as_float(raw[4 * th + 2]));
@@ -930,7 +933,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                 }
                 sfor<4 * k, 4 * k + 4>([&](auto i_) { pf_load(pf_next, i_); });
                 if constexpr (k == 7) {
-                    if (bpsk) cw_pf = __ldg(P.Cbits + (long long)(has_next ? p_next : p) * 512 + wa * 32 + lane);
+                    if constexpr (!IDC) {
+                        if (bpsk) cw_pf = __ldg(P.Cbits + (long long)(has_next ? p_next : p) * 512 + wa * 32 + lane);
+                    }
                 }
             }
         });
