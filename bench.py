@@ -149,9 +149,10 @@ def cpu_oracle_sample(w, V, C, target_s=12.0, steps=1):
     cores = oracle.max_threads()
     # calibrate with all threads busy: `cores` gates x a few IPPs
     pc = min(4, w.n_ipp)
-    t0 = time.perf_counter()
-    oracle.spectra(V[:pc], C[:pc], N=w.N, n_ranges=min(cores, w.n_ranges), r0=w.r0, stride=w.stride)
-    per_round = (time.perf_counter() - t0) / pc * w.n_ipp        # seconds for `cores` gates x all IPPs
+    for _ in range(2):                                           # the first call also starts the OpenMP team
+        t0 = time.perf_counter()
+        oracle.spectra(V[:pc], C[:pc], N=w.N, n_ranges=min(cores, w.n_ranges), r0=w.r0, stride=w.stride)
+        per_round = (time.perf_counter() - t0) / pc * w.n_ipp    # seconds for `cores` gates x all IPPs
     rounds = int(max(1, target_s / max(per_round, 1e-9)))
     gates = min(w.n_ranges, rounds * cores)
     times = []
