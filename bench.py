@@ -326,6 +326,26 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+def probe_mem():
+    """what an SM and the chip can move to and from L2 / DRAM (GB/s, 128-bit accesses)."""
+    import torch
+    from paper_2311_18737_b200 import binding as pl
+    torch.cuda.set_device(0)
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    kinds = {"read": 0, "write": 1, "copy": 2, "tma_store": 3}
+    out = {"probe": "plspec_diag_mem_bandwidth", "unit": "GB/s", "n_sm": n_sm, "rows": []}
+    for mb, passes in ((32, 64), (64, 32), (2048, 2)):
+        for ctas in (1, 8, n_sm, 2 * n_sm, 4 * n_sm):
+            if mb == 2048 and ctas < n_sm:
+                continue
+            row = {"buffer_MiB": mb, "ctas": ctas}
+            for name, kind in kinds.items():
+                p = max(1, passes // 16) if ctas < n_sm else passes
+                row[name] = round(pl.plspec_diag_mem_bandwidth(kind, mb << 20, ctas, p), 1)
+            out["rows"].append(row)
+    print(json.dumps(out), flush=True)
+
+
 # ------------------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
@@ -338,6 +358,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT comparison pipeline")
     ap.add_argument("--no-peak", action="store_true", help="skip the FP32 peak micro-benchmark")
+    ap.add_argument("--probe-mem", action="store_true",
+                    help="print the device's streaming bandwidths (plspec_diag_mem_bandwidth: L2-resident and DRAM-sized "
+                         "buffers, reads / writes / copy / TMA stores, 1 ... 4 CTAs per SM) as one JSON line and exit")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 fused")
     ap.add_argument("--chunks", type=int, default=0)
     ap.add_argument("--shard", default="replicas", choices=["replicas", "ipp", "gates"],
@@ -358,6 +381,8 @@ def main():
         w = synth.scaled(w, n_ranges=args.n_ranges or None, n_ipp=args.n_ipp or None, ipp_len=w.ipp_len)
     if args.impl == "reference":
         return run_reference(args, w)
+    if args.probe_mem:
+        return probe_mem()
     args.warmup = max(args.warmup, 3)
 
     import torch

@@ -134,7 +134,11 @@ int plspec_accumulate(plspec_handle h, const void *voltages, const void *codes,
  * Finish an integration: wait for all accumulate work, write S_out[n_ranges][N] (fp32,
  * row-major, natural FFT bin order, un-normalised sum) and zero the accumulators so the next
  * integration starts clean ("Upon completion, we transfer the spectrum result
- * back").  S_out is [host|device]; the call blocks until S_out is complete.
+ * back").  S_out is [host|device]; the call blocks until S_out is complete.  The work is enqueued on the stream of the
+ * latest plspec_accumulate (plspec_reset and plspec_finalize_products likewise): that stream must still exist.
+ * Host S_out: the deferred pulses of a host-buffer call (PLSPEC_OPT_DEFER) are transformed here, one gate range after
+ * the other, and each finished range is copied out while the next one computes; pinned memory makes those copies
+ * asynchronous.
  */
 int plspec_finalize(plspec_handle h, float *S_out);
 
@@ -216,6 +220,20 @@ int plspec_finalize_products(plspec_handle h, float *S_out, const plspec_product
  * Errors: PLSPEC_ERR_INVALID_ARG, PLSPEC_ERR_ALLOC, PLSPEC_ERR_CUDA.  Needs no handle; touches no integrator state.
  */
 int plspec_diag_fp32_peak(int packed, int iters, int reps, double *tflops_best, double *tflops_mean, void *stream);
+
+/*
+ * DIAGNOSTIC (the N > 16384 paths): streaming bandwidth of the current device with 128-bit
+ * accesses, the figures behind the scratch-versus-ring argument.  `n_ctas` CTAs of 512 threads each walk a buffer of
+ * `bytes` bytes (allocated and freed by the call, rounded down to whole MiB) `passes` times; one warm-up launch, then
+ * the fastest of three launches, timed with CUDA events on `stream`; the call blocks.  A buffer well below the L2 size
+ * (126 MB on B200) measures the SM <-> L2 paths, a buffer of gigabytes DRAM.
+ *   kind   0 = read (ld.global.cg), 1 = write (st.global), 2 = copy first half -> second half (bytes read + written
+ *          are counted), 3 = write by the TMA engine (cp.async.bulk stores of 16 KB from shared memory, 4 in flight)
+ *   bytes  1 MiB ... 8 GiB;  n_ctas 1 ... 65535 (148 = one per SM);  passes >= 1
+ *   gbs    [host] bandwidth in GB/s
+ * Errors: PLSPEC_ERR_INVALID_ARG, PLSPEC_ERR_ALLOC, PLSPEC_ERR_CUDA.  Needs no handle.
+ */
+int plspec_diag_mem_bandwidth(int kind, long long bytes, int n_ctas, int passes, double *gbs, void *stream);
 
 /* EXTENSIONS ------------------------------------------------------------------------------- */
 int plspec_reset(plspec_handle h);                        /* zero the accumulators, no output */

@@ -42,7 +42,7 @@ LIB_PATH = os.path.join(_HERE, "libplspec.so")
 EXPORTED_SYMBOLS = (
     "plspec_create", "plspec_accumulate", "plspec_finalize", "plspec_reset", "plspec_destroy",
     "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_profile", "plspec_mean_spectrum",
-    "plspec_diag_fp32_peak", "plspec_finalize_products",
+    "plspec_diag_fp32_peak", "plspec_diag_mem_bandwidth", "plspec_finalize_products",
     "plspec_strerror",
     "plspec_version",
 )
@@ -105,6 +105,7 @@ def lib() -> ctypes.CDLL:
         L.plspec_profile.argtypes = [vp, ci, ci, ci, ci, ci, vp, vp, vp, vp, vp, vp]
         L.plspec_mean_spectrum.argtypes = [vp, vp, ci, ci, ci, ci, vp]
         L.plspec_finalize_products.argtypes = [vp, vp, ctypes.POINTER(plspec_products_t)]
+        L.plspec_diag_mem_bandwidth.argtypes = [ci, ctypes.c_longlong, ci, ci, ctypes.POINTER(ctypes.c_double), vp]
         L.plspec_diag_fp32_peak.argtypes = [ci, ci, ci, ctypes.POINTER(ctypes.c_double),
                                             ctypes.POINTER(ctypes.c_double), vp]
         for name in _INT_STATUS:
@@ -193,6 +194,14 @@ def plspec_diag_fp32_peak(packed=True, iters=1 << 16, reps=10, stream=None) -> d
     _check(None, lib().plspec_diag_fp32_peak(int(bool(packed)), int(iters), int(reps), ctypes.byref(best),
                                              ctypes.byref(mean), _stream_ptr(stream)), "plspec_diag_fp32_peak")
     return {"tflops_best": best.value, "tflops_mean": mean.value}
+
+
+def plspec_diag_mem_bandwidth(kind, n_bytes, n_ctas, passes=8, stream=None) -> float:
+    """Streaming bandwidth in GB/s (kind: 0 read, 1 write, 2 copy, 3 TMA bulk stores); see include/plspec.h."""
+    gbs = ctypes.c_double()
+    _check(None, lib().plspec_diag_mem_bandwidth(int(kind), int(n_bytes), int(n_ctas), int(passes), ctypes.byref(gbs),
+                                                 _stream_ptr(stream)), "plspec_diag_mem_bandwidth")
+    return gbs.value
 
 
 def plspec_reset(h) -> None:

@@ -1052,6 +1052,52 @@ int plspec_diag_fp32_peak(int packed, int iters, int reps, double *tflops_best, 
     return PLSPEC_OK;
 }
 
+int plspec_diag_mem_bandwidth(int kind, long long bytes, int n_ctas, int passes, double *gbs, void *stream_) {
+    if (kind < 0 || kind > 3 || bytes < (1 << 20) || bytes > (8LL << 30) || n_ctas < 1 || n_ctas > 65535 || passes < 1 || !gbs)
+        return PLSPEC_ERR_INVALID_ARG;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    bytes &= ~((long long)(1 << 20) - 1);                              // whole MiB
+    unsigned char *buf = nullptr;
+    uint4 *sink = nullptr;
+    if (cudaMalloc((void **)&buf, (size_t)bytes) != cudaSuccess || cudaMalloc((void **)&sink, sizeof(uint4)) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (buf) cudaFree(buf);
+        return PLSPEC_ERR_ALLOC;
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = PLSPEC_OK;
+    if (cudaMemsetAsync(buf, 0, (size_t)bytes, stream) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess ||
+        cudaEventCreate(&e1) != cudaSuccess)
+        rc = PLSPEC_ERR_CUDA;
+    const size_t nvec = (size_t)bytes / 16;
+    double moved = (double)bytes * passes;                             // bytes read + written by one launch
+    if (kind == 3) moved = (double)(((size_t)bytes / n_ctas) & ~(size_t)16383) * n_ctas * passes;
+    double best_ms = 0.0;
+    for (int r = -1; r < 3 && rc == PLSPEC_OK; r++) {                  // r = -1: warm-up (also brings the buffer into L2)
+        cudaEventRecord(e0, stream);
+        switch (kind) {
+            case 0: bw_read_kernel<<<n_ctas, 512, 0, stream>>>((const uint4 *)buf, nvec, passes, sink); break;
+            case 1: bw_write_kernel<<<n_ctas, 512, 0, stream>>>((uint4 *)buf, nvec, passes); break;
+            case 2: bw_copy_kernel<<<n_ctas, 512, 0, stream>>>((uint4 *)buf, nvec, passes); break;
+            default: bw_tma_store_kernel<<<n_ctas, 512, 0, stream>>>(buf, (size_t)bytes, passes); break;
+        }
+        cudaEventRecord(e1, stream);
+        float ms = 0.f;
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess || ms <= 0.f) {
+            rc = PLSPEC_ERR_CUDA;
+            break;
+        }
+        if (r >= 0 && (best_ms == 0.0 || ms < best_ms)) best_ms = ms;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf);
+    cudaFree(sink);
+    if (rc != PLSPEC_OK) { (void)cudaGetLastError(); return rc; }
+    *gbs = moved / (best_ms * 1e-3) / 1e9;
+    return PLSPEC_OK;
+}
+
 int plspec_reset(plspec_handle h) {
     if (!h) return PLSPEC_ERR_INVALID_ARG;
     cudaStream_t st = h->last_stream;

@@ -533,3 +533,17 @@ def test_ring_mode_rounds(N, R, dtype, L, stride, depth, ahead):
                 it.finalize(out)
                 m = gate_metric(out.cpu().numpy(), S_ref)
                 assert m.max() <= TOL, f"stage {stage}: worst gate {int(m.argmax())}: {m.max():.3e}"
+
+
+# ---- diagnostics (the measured roofline denominators) -------------------------------------------------------------
+def test_diagnostic_calls():
+    pk = pl.plspec_diag_fp32_peak(packed=True, iters=1 << 12, reps=3)
+    assert 10.0 < pk["tflops_mean"] <= pk["tflops_best"] < 200.0
+    for kind in (0, 1, 2, 3):
+        gbs = pl.plspec_diag_mem_bandwidth(kind, 32 << 20, 148, passes=4)
+        assert 200.0 < gbs < 50000.0, (kind, gbs)
+    for bad in (dict(kind=4), dict(n_bytes=1000), dict(n_ctas=0), dict(passes=0)):
+        args = {**dict(kind=0, n_bytes=32 << 20, n_ctas=8, passes=1), **bad}
+        with pytest.raises(pl.PlspecError) as e:
+            pl.plspec_diag_mem_bandwidth(**args)
+        assert e.value.status == pl.PLSPEC_ERR_INVALID_ARG

@@ -166,7 +166,7 @@ def test_products_on_a_user_stream_and_misaligned_profile_input():
 @pytest.mark.parametrize("N,R,dtype,kernel", [(1024, 19, synth.CF32, pl.KERNEL_FUSED), (4096, 11, synth.SC16, pl.KERNEL_FUSED),
                                               (16384, 5, synth.SC16, pl.KERNEL_FUSED), (65536, 3, synth.CF32, pl.KERNEL_FUSED),
                                               (32768, 3, synth.SC16, pl.KERNEL_FUSED), (256, 9, synth.CF32, pl.KERNEL_GENERIC),
-                                              (2048, 7, synth.CF32, pl.KERNEL_GENERIC)])
+                                              (2048, 7, synth.CF32, pl.KERNEL_GENERIC), (32768, 2, synth.CF32, pl.KERNEL_GENERIC)])
 def test_finalize_products_equals_finalize_then_products(N, R, dtype, kernel):
     """One pass: S_out must be the spectrum the oracle computes, and the mean spectrum / line search must be exactly
     what their oracles give ON THAT S_out (bins, powers, mean bit for bit; noise floor to summation order)."""
