@@ -574,9 +574,20 @@ int flush_tail(plspec_ctx *h, cudaStream_t stream) {
 int accumulate_from_host(plspec_ctx *h, const void *V, const void *C, int n_ipp, cudaStream_t stream) {
     const size_t esz = h->dtype == PLSPEC_SC16 ? 4 : 8;
     const size_t per_ipp = (size_t)h->span * esz + (h->opt_shared_code ? 0 : (size_t)h->L * sizeof(float2));
-    // the second half of the call's IPPs (as far as they fit kTailMaxBytes) is staged but left for plspec_finalize
+    // the last part of the call's IPPs (as far as they fit kTailMaxBytes) is staged but left for plspec_finalize
     // (or the next plspec_accumulate): see struct Tail
-    int n_tail = h->opt_defer ? n_ipp - n_ipp / 2 : 0;
+    // How many: half, or more where the write-out is long against the transform (large N, few pulses): the deferred
+    // transform should last ~1.3x the device -> host copy of S that hides under it.  Estimates: 5 N log2 N flop per
+    // window at half the FP32 peak; 50 GB/s for the copy.
+    double frac = 0.5;
+    {
+        const double t_d2h = (double)h->R * h->N * 4.0 / 50e9;
+        const double t_all = (double)n_ipp * h->R * 5.0 * h->N * (double)ilog2(h->N) / 37e12;
+        const double want = 1.3 * t_d2h / (t_all > 0 ? t_all : 1.0);
+        frac = want < 0.5 ? 0.5 : (want > 0.75 ? 0.75 : want);
+    }
+    int n_tail = h->opt_defer ? (int)(n_ipp * frac + 0.999) : 0;
+    if (n_tail > n_ipp) n_tail = n_ipp;
     const size_t tail_cap = kTailMaxBytes / per_ipp;
     if ((size_t)n_tail > tail_cap) n_tail = (int)tail_cap;
     const int n_head = n_ipp - n_tail;
@@ -857,23 +868,39 @@ int plspec_finalize(plspec_handle h, float *S_out) {
         (void)cudaGetLastError();
         return PLSPEC_ERR_ALLOC;
     }
-    // Gate ranges.  Device S_out: one.  Host S_out: up to kMaxRanges of >= ~8 MB each; range k is transformed (the
-    // deferred IPPs, if any), un-permuted into S_tmp and copied out on the d2h stream while range k + 1 computes.
-    int n_ranges = 1;
-    if (!out_dev) {
-        const size_t want = total * sizeof(float) / ((size_t)8 << 20);
-        n_ranges = want < 1 ? 1 : (want > (size_t)kMaxRanges ? kMaxRanges : (int)want);
-    }
+    // Gate ranges.  Device S_out: one.  Host S_out: up to kMaxRanges of >= ~8 MB; range k is transformed (the deferred
+    // IPPs, if any), un-permuted into S_tmp and copied out on the d2h stream while range k + 1 computes.  Equal ranges
+    // keep the copy stream and the kernels in step (where the copy of S takes about as long as the deferred transform,
+    // cfg 4, a small first range leaves the copy stream waiting for the large second one); only the last range is
+    // smaller (S / 16, within 2 ... 8 MB): its copy is the part nothing overlaps.
     const int n_groups = (h->R + h->gates_per_cta - 1) / h->gates_per_cta;
-    if (n_ranges > n_groups) n_ranges = n_groups;
+    int n_ranges = 1;
+    int bound[kMaxRanges + 1];                            // gate groups: range k = [bound[k], bound[k + 1])
+    bound[0] = 0;
+    if (!out_dev) {
+        const double s_bytes = (double)total * sizeof(float), mb = (double)(1 << 20);
+        const size_t want = (size_t)(s_bytes / (8 * mb));
+        n_ranges = want < 1 ? 1 : (want > (size_t)kMaxRanges ? kMaxRanges : (int)want);
+        if (n_ranges > n_groups) n_ranges = n_groups;
+        double last = 1.0 / n_ranges;                     // fraction of the gates in the last range
+        if (n_ranges >= 4) {
+            double edge = s_bytes / 16;
+            edge = edge < 2 * mb ? 2 * mb : (edge > 8 * mb ? 8 * mb : edge);
+            if (edge / s_bytes < last) last = edge / s_bytes;
+        }
+        for (int k = 1; k < n_ranges; k++) bound[k] = (int)((1.0 - last) * n_groups * k / (n_ranges - 1) + 0.5);
+        for (int k = 1; k < n_ranges; k++)                // strictly increasing, inside (0, n_groups)
+            if (bound[k] <= bound[k - 1] || bound[k] >= n_groups) { n_ranges = 1; break; }
+    }
+    bound[n_ranges] = n_groups;
     Tail &t = h->tail;
     const bool tail = t.pending;
     t.pending = false;
     const int RAe = h->kind == 2 ? h->RA : 1, NC = h->kind == 2 ? 1024 : h->Nk, M = h->Q * RAe;
     const int TC = 4096 / M < NC ? 4096 / M : NC;
     for (int k = 0; k < n_ranges; k++) {
-        const int g_lo = (int)((long long)n_groups * k / n_ranges) * h->gates_per_cta;
-        int g_hi = (int)((long long)n_groups * (k + 1) / n_ranges) * h->gates_per_cta;
+        const int g_lo = bound[k] * h->gates_per_cta;
+        int g_hi = bound[k + 1] * h->gates_per_cta;
         if (g_hi > h->R) g_hi = h->R;
         const int g_cnt = g_hi - g_lo;
         const size_t off = (size_t)g_lo * (size_t)h->N, cnt = (size_t)g_cnt * (size_t)h->N;
