@@ -1084,6 +1084,7 @@ int plspec_diag_mem_bandwidth(int kind, long long bytes, int n_ctas, int passes,
         return PLSPEC_ERR_INVALID_ARG;
     cudaStream_t stream = (cudaStream_t)stream_;
     bytes &= ~((long long)(1 << 20) - 1);                              // whole MiB
+    if (kind == 3 && bytes / n_ctas < 16384) return PLSPEC_ERR_INVALID_ARG;   // a CTA's share: at least one bulk store
     unsigned char *buf = nullptr;
     uint4 *sink = nullptr;
     if (cudaMalloc((void **)&buf, (size_t)bytes) != cudaSuccess || cudaMalloc((void **)&sink, sizeof(uint4)) != cudaSuccess) {
