@@ -74,3 +74,20 @@ def test_header_and_binding_constants_agree():
     for name in ("PLSPEC_OPT_KERNEL", "PLSPEC_OPT_IPP_CHUNKS", "PLSPEC_OPT_H2D_BATCH", "PLSPEC_OPT_BPSK_PACK",
                  "PLSPEC_OPT_STAGE", "PLSPEC_OPT_SPLIT", "PLSPEC_OPT_SHARED_CODE"):
         assert getattr(pl, name) == consts[name], name
+
+
+def test_handle_free_calls_check_their_arguments_before_touching_the_device(lib):
+    """Argument errors of the diagnostic / product calls come first, with or without a GPU."""
+    d = ctypes.c_double()
+    vp = ctypes.c_void_p
+    assert lib.plspec_diag_fp32_peak(2, 1, 1, ctypes.byref(d), ctypes.byref(d), None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_diag_fp32_peak(1, 0, 1, ctypes.byref(d), ctypes.byref(d), None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_diag_fp32_peak(1, 1, 1, None, ctypes.byref(d), None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_diag_mem_bandwidth(9, 1 << 25, 8, 1, ctypes.byref(d), None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_diag_mem_bandwidth(0, 1000, 8, 1, ctypes.byref(d), None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_diag_mem_bandwidth(0, 1 << 25, 8, 1, None, None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_finalize_products(None, None, None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_profile(None, 4, 1024, 1, 1, 0, None, None, None, None, None, None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_mean_spectrum(None, None, 4, 1024, 1, 0, None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_configure(None, pl.PLSPEC_OPT_SPLIT, 1) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_get_stats(None, None) == pl.PLSPEC_ERR_INVALID_ARG and lib.plspec_reset(None) == pl.PLSPEC_ERR_INVALID_ARG

@@ -1,6 +1,7 @@
 """Randomised parity: seeded random problem shapes, code families, buffer kinds and library options through the C ABI
 against the float64 oracle on every gate (bar 1e-4, BASELINE.json north_star).  The default run is a few dozen cases
-(about a minute on a B200); PLSPEC_FUZZ_CASES=<n> widens it for a soak run (profiles/r02_fuzz.md)."""
+(about a minute on a B200); PLSPEC_FUZZ_CASES=<n> widens it for a soak run, PLSPEC_FUZZ_SEED / PLSPEC_FUZZ_BUDGET / PLSPEC_FUZZ_MAX_IPP vary the
+sequence and the problem sizes (profiles/r02_fuzz.md)."""
 import os
 
 import numpy as np
@@ -15,7 +16,9 @@ pytestmark = pytest.mark.gpu
 
 TOL = 1e-4
 N_CASES = int(os.environ.get("PLSPEC_FUZZ_CASES", "48"))
-BUDGET = 3.0e7          # decoded samples per case (P * R * N): keeps the oracle at a fraction of a second
+SEED = int(os.environ.get("PLSPEC_FUZZ_SEED", "20260105"))
+BUDGET = float(os.environ.get("PLSPEC_FUZZ_BUDGET", "3.0e7"))   # decoded samples per case (P * R * N): keeps the oracle at a fraction of a second
+MAX_IPP = int(os.environ.get("PLSPEC_FUZZ_MAX_IPP", "8"))
 
 
 def draw_case(rng):
@@ -24,9 +27,9 @@ def draw_case(rng):
     L = int(N if rng.random() < 0.5 else rng.integers(1, N + 1))
     stride = int(rng.choice([1, 1, 2, 3, 4, 7, 25, 64]))
     r0 = int(rng.integers(0, 9))
-    P = int(rng.integers(1, 9))
+    P = int(rng.integers(1, MAX_IPP + 1))
     r_max = max(1, int(BUDGET / (P * N)))
-    R = int(rng.integers(1, min(r_max, 300) + 1))
+    R = int(rng.integers(1, min(r_max, 300 if BUDGET <= 3.0e7 else 2000) + 1))
     pad = int(rng.choice([0, 0, 1, 5, 100]))
     M = r0 + (R - 1) * stride + L + pad
     dtype = int(rng.integers(0, 2))
@@ -96,7 +99,7 @@ def run_case(c):
 
 
 def test_random_cases_against_the_oracle():
-    rng = np.random.default_rng(20260105)
+    rng = np.random.default_rng(SEED)
     worst, worst_case = 0.0, ""
     for k in range(N_CASES):
         c = draw_case(rng)
