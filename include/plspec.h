@@ -164,6 +164,23 @@ int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, in
                    int *k_up, float *p_up, int *k_dn, float *p_dn, float *noise, void *stream);
 
 /*
+ * EXTENSION: plspec_profile for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc).  Same arguments, same five outputs (k_up, p_up, k_dn, p_dn equal
+ * plspec_profile's bit for bit; noise to float64 summation order, ~1e-7 relative), computed by a (gate, column tile)
+ * grid whose CTAs meet in a 32-byte workspace per gate.  That workspace is a file-scope array in device memory
+ * (csrc/plspec_static.cu) of PLSPEC_STATIC_MAX_GATES entries: 256 KiB that every GPU which loads the library holds
+ * until the process exits.  The call makes no cudaMalloc / cudaFree and calls no allocating library routine; it
+ * enqueues one memset (clearing the entries it uses) and one kernel on `stream` and returns without synchronising.
+ *   n_ranges  1 ... PLSPEC_STATIC_MAX_GATES; more is PLSPEC_ERR_INVALID_ARG (use plspec_profile)
+ * All calls, on every stream and from every thread, SHARE the one workspace of the device: two calls that overlap
+ * on the GPU race on it and their outputs are undefined.  Calls on one stream, or ordered by events, are safe.
+ * Errors: as plspec_profile, plus PLSPEC_ERR_UNSUPPORTED (device is not sm_100).  Needs no handle.
+ */
+#define PLSPEC_STATIC_MAX_GATES 8192
+int plspec_profile_static(const float *S, int n_ranges, int N, int n_ipp, int k_min, int guard,
+                          int *k_up, float *p_up, int *k_dn, float *p_dn, float *noise, void *stream);
+
+/*
  * EXTENSION ("mean P = S/P (Eq. 8), optional fftshift"): the mean power spectrum of a
  * finished integration, PAPER.md:79 (Eq. 8: the estimate is the AVERAGE <|x|^2>; the hot path keeps the plain
  * sum, reading A2), optionally with zero frequency moved to the middle of every row.

@@ -42,7 +42,7 @@ LIB_PATH = os.path.join(_HERE, "libplspec.so")
 EXPORTED_SYMBOLS = (
     "plspec_create", "plspec_accumulate", "plspec_finalize", "plspec_reset", "plspec_destroy",
     "plspec_configure", "plspec_get_stats", "plspec_last_cuda_error", "plspec_profile", "plspec_mean_spectrum",
-    "plspec_diag_fp32_peak", "plspec_diag_mem_bandwidth", "plspec_finalize_products",
+    "plspec_diag_fp32_peak", "plspec_diag_mem_bandwidth", "plspec_finalize_products", "plspec_profile_static",
     "plspec_strerror",
     "plspec_version",
 )
@@ -103,6 +103,7 @@ def lib() -> ctypes.CDLL:
         L.plspec_strerror.restype = ctypes.c_char_p
         L.plspec_version.restype = ctypes.c_char_p
         L.plspec_profile.argtypes = [vp, ci, ci, ci, ci, ci, vp, vp, vp, vp, vp, vp]
+        L.plspec_profile_static.argtypes = [vp, ci, ci, ci, ci, ci, vp, vp, vp, vp, vp, vp]
         L.plspec_mean_spectrum.argtypes = [vp, vp, ci, ci, ci, ci, vp]
         L.plspec_finalize_products.argtypes = [vp, vp, ctypes.POINTER(plspec_products_t)]
         L.plspec_diag_mem_bandwidth.argtypes = [ci, ctypes.c_longlong, ci, ci, ctypes.POINTER(ctypes.c_double), vp]
@@ -181,6 +182,17 @@ def plspec_profile(S, n_ranges, N, n_ipp, k_min, guard, k_up, p_up, k_dn, p_dn, 
     _check(None, lib().plspec_profile(_ptr(S), int(n_ranges), int(N), int(n_ipp), int(k_min), int(guard), _ptr(k_up),
                                       _ptr(p_up), _ptr(k_dn), _ptr(p_dn), _ptr(noise), _stream_ptr(stream)),
            "plspec_profile")
+
+
+STATIC_MAX_GATES = 8192                       # PLSPEC_STATIC_MAX_GATES of include/plspec.h
+
+
+def plspec_profile_static(S, n_ranges, N, n_ipp, k_min, guard, k_up, p_up, k_dn, p_dn, noise, stream=None) -> None:
+    """plspec_profile without any device allocation (file-scope workspace, n_ranges <= STATIC_MAX_GATES; calls that
+    overlap on the GPU race on it -- include/plspec.h)."""
+    _check(None, lib().plspec_profile_static(_ptr(S), int(n_ranges), int(N), int(n_ipp), int(k_min), int(guard),
+                                             _ptr(k_up), _ptr(p_up), _ptr(k_dn), _ptr(p_dn), _ptr(noise),
+                                             _stream_ptr(stream)), "plspec_profile_static")
 
 
 def plspec_mean_spectrum(S, P_out, n_ranges, N, n_ipp, centred=False, stream=None) -> None:

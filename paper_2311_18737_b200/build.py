@@ -1,6 +1,7 @@
 """Build the CUDA libraries (sm_100a) in-tree with nvcc.  `python -m paper_2311_18737_b200.build`.
 
-libplspec.so        the product: the C ABI of include/plspec.h (no cuFFT, no cuBLAS)
+libplspec.so        the product: the C ABI of include/plspec.h (no cuFFT, no cuBLAS); plspec_api.cu + plspec_static.cu
+                    (the entry point that allocates nothing, with its file-scope device workspace)
 libplspec_cufft.so  comparison point only (csrc/cufft_pipeline.cu: the paper's multiply -> cuFFT -> accumulate
                     structure); loaded by bench.py alone, never by the binding
 """
@@ -15,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libplspec.so")
 LIB_CUFFT = os.path.join(HERE, "libplspec_cufft.so")
-SOURCES = ["plspec_api.cu"]
+SOURCES = ["plspec_api.cu", "plspec_static.cu"]
 HEADERS = ["plspec_common.cuh", "plspec_kernels.cuh", "plspec_fused.cuh", os.path.join("..", "..", "include", "plspec.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
