@@ -89,5 +89,10 @@ def test_handle_free_calls_check_their_arguments_before_touching_the_device(lib)
     assert lib.plspec_finalize_products(None, None, None) == pl.PLSPEC_ERR_INVALID_ARG
     assert lib.plspec_profile(None, 4, 1024, 1, 1, 0, None, None, None, None, None, None) == pl.PLSPEC_ERR_INVALID_ARG
     assert lib.plspec_mean_spectrum(None, None, 4, 1024, 1, 0, None) == pl.PLSPEC_ERR_INVALID_ARG
+    assert lib.plspec_profile_static(None, 4, 1024, 1, 1, 0, None, None, None, None, None, None) == pl.PLSPEC_ERR_INVALID_ARG
+    one = ctypes.c_float()                              # size beyond the static workspace: refused before any CUDA call
+    ptrs = [ctypes.cast(ctypes.byref(one), vp)] * 5
+    assert lib.plspec_profile_static(ctypes.cast(ctypes.byref(one), vp), pl.STATIC_MAX_GATES + 1, 1024, 1, 1, 0, *ptrs,
+                                     None) == pl.PLSPEC_ERR_INVALID_ARG
     assert lib.plspec_configure(None, pl.PLSPEC_OPT_SPLIT, 1) == pl.PLSPEC_ERR_INVALID_ARG
     assert lib.plspec_get_stats(None, None) == pl.PLSPEC_ERR_INVALID_ARG and lib.plspec_reset(None) == pl.PLSPEC_ERR_INVALID_ARG
