@@ -254,6 +254,12 @@ def products_timing(w, S_dev, flush, reps=7, it=None, accumulate=None):
              "profile": (4, lambda: pl.plspec_profile(S_dev, R, N, w.n_ipp, max(1, N // 256), 2, ki[0], pf[0], ki[1],
                                                       pf[1], pf[2]))}
     out = {"hbm_peak_gbs": peak, "peak_source": src}
+    # two yardsticks under the very same timing: the smallest launch this library has (plspec_profile of one 16-bin
+    # gate: what the two events see of a launch that moves nothing) and a plain library pass over S (torch.sum: 4 B per
+    # bin, no search): context for what a one-pass product of this size can reach between two events
+    S1 = torch.ones((1, 16), dtype=torch.float32, device="cuda")
+    calls["empty_launch"] = (0, lambda: pl.plspec_profile(S1, 1, 16, 1, 1, 0, ki[0], pf[0], ki[1], pf[1], pf[2]))
+    calls["read_pass_torch_sum"] = (4, lambda: S_dev.sum())
     for name, (bpb, call) in calls.items():
         ts = []
         for _ in range(reps + 2):

@@ -1013,7 +1013,7 @@ int plspec_profile(const float *S, int n_ranges, int N, int n_ipp, int k_min, in
         if (a.type != cudaMemoryTypeDevice && a.type != cudaMemoryTypeManaged) return PLSPEC_ERR_INVALID_ARG;
     }
     if ((uintptr_t)S & 15) return PLSPEC_ERR_INVALID_ARG;  // rows are read in 128-bit loads
-    profile_kernel<<<(unsigned)n_ranges, 256, 0, (cudaStream_t)stream>>>(S, N, n_ipp, k_min, guard, k_up, p_up, k_dn,
+    profile_kernel<<<(unsigned)n_ranges, kProfileThreads, 0, (cudaStream_t)stream>>>(S, N, n_ipp, k_min, guard, k_up, p_up, k_dn,
                                                                          p_dn, noise);
     if (cudaGetLastError() != cudaSuccess) return PLSPEC_ERR_CUDA;
     return PLSPEC_OK;

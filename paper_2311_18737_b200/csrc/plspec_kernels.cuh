@@ -249,28 +249,32 @@ __global__ void __launch_bounds__(256) predecode_kernel(const KParams P, float2 
 // Post-integration products per range gate (SURVEY.md 8(f) NEXT-2; PAPER.md:40-45 Eq. 1, :79 Eq. 8):
 // arg max of S over the up-shifted half [k_min, N/2) and the down-shifted half (N/2, N - k_min] (lowest bin
 // wins a tie), the mean power S / n_ipp at those bins, and the mean of the remaining bins of
-// [k_min, N - k_min] \ {N/2} further than `guard` from either line (float64 sum).  One CTA per gate.
+// [k_min, N - k_min] \ {N/2} further than `guard` from either line (float64 sum).  One CTA of 128 threads per gate.
 struct ProfileBest { float v; int k; };
 __device__ __forceinline__ ProfileBest better(ProfileBest a, ProfileBest b) {
     return (b.v > a.v || (b.v == a.v && b.k < a.k)) ? b : a;
 }
-__global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ S, int N, int n_ipp, int k_min, int guard,
-                                                      int *__restrict__ k_up, float *__restrict__ p_up,
-                                                      int *__restrict__ k_dn, float *__restrict__ p_dn,
-                                                      float *__restrict__ noise) {
-    // One pass over the row in 128-bit loads (eight in flight per thread): both arg maxima and the float64 sum of
-    // every searched bin; the few bins within `guard` of the lines are then taken out of the sum again (they are
-    // still in L1/L2), so the row crosses HBM once.
-    __shared__ ProfileBest sb[2][8];
-    __shared__ double ssum[8];
-    __shared__ int scnt[8];
+constexpr int kProfileThreads = 128;
+__global__ void __launch_bounds__(kProfileThreads) profile_kernel(const float *__restrict__ S, int N, int n_ipp, int k_min, int guard,
+                                                                  int *__restrict__ k_up, float *__restrict__ p_up,
+                                                                  int *__restrict__ k_dn, float *__restrict__ p_dn,
+                                                                  float *__restrict__ noise) {
+    // One pass over the row in 128-bit loads, software pipelined: the four loads of the next batch are in flight while
+    // this batch is searched (against 256 threads x 8 loads and no overlap: 2-10 % faster on the bench shapes,
+    // DESIGN.md section 7): both arg maxima and the float64 sum of every searched bin; the few bins within `guard` of
+    // the lines are then taken out of the sum again (they are still in L1/L2), so the row crosses HBM once.
+    constexpr int T = kProfileThreads, W = T / 32, U = 4;
+    __shared__ ProfileBest sb[2][W];
+    __shared__ double ssum[W];
+    __shared__ int scnt[W];
     __shared__ int sk[2];
     __shared__ double stotal;
     const float *row = S + (long long)blockIdx.x * N;
     const float4 *row4 = reinterpret_cast<const float4 *>(row);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lo = k_min, hi = N - k_min, mid = N / 2, nv = N / 4;
-    ProfileBest up = {-1.f, 0x7fffffff}, dn = {-1.f, 0x7fffffff};      // S >= 0: any bin beats the start value
+    const ProfileBest none = {-1.f, 0x7fffffff};                       // S >= 0: any bin beats the start value
+    ProfileBest up = none, dn = none;
     double acc = 0.0;
     auto take = [&](float v, int f) {
         if (f >= lo && f <= hi && f != mid) {
@@ -279,20 +283,20 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
             acc += (double)v;
         }
     };
-    for (int i0 = tid; i0 < nv; i0 += 8 * 256) {
-        float4 v[8];
+    auto load = [&](int i) { return i < nv ? __ldg(row4 + i) : make_float4(0.f, 0.f, 0.f, 0.f); };
+    float4 v[U], nx[U];
 #pragma unroll
-        for (int u = 0; u < 8; u++) {
-            const int i = i0 + u * 256;
-            v[u] = i < nv ? __ldg(row4 + i) : make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-        // interior vectors: the four bins summed in float32, the eight vectors of a batch pairwise in float32 (32 bins:
-        // five roundings of 2^-24 relative, against the 1e-6 the noise floor is good to), everything above in float64
-        // -- float64 adds are scarce on this part
-        float fs[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    for (int u = 0; u < U; u++) v[u] = load(tid + u * T);
+    for (int i0 = tid; i0 < nv; i0 += U * T) {
 #pragma unroll
-        for (int u = 0; u < 8; u++) {
-            const int i = i0 + u * 256;
+        for (int u = 0; u < U; u++) nx[u] = load(i0 + (U + u) * T);
+        // interior vectors: the four bins summed in float32, the four vectors of a batch too (16 bins: at most five
+        // roundings of 2^-24 relative on any path, against the 1e-6 the noise floor is good to), everything above in
+        // float64
+        float fs = 0.f;
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int i = i0 + u * T;
             if (i >= nv) continue;
             const int f0 = 4 * i;
             if (f0 >= lo && f0 + 3 <= hi && (f0 + 3 < mid || f0 > mid)) {   // interior vector: one candidate, one add
@@ -301,37 +305,48 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
                 if (v[u].z > c.v) c = {v[u].z, f0 + 2};
                 if (v[u].w > c.v) c = {v[u].w, f0 + 3};
                 if (f0 < mid) up = better(up, c); else dn = better(dn, c);
-                fs[u] = (v[u].x + v[u].y) + (v[u].z + v[u].w);
+                fs += (v[u].x + v[u].y) + (v[u].z + v[u].w);
             } else {
                 take(v[u].x, f0); take(v[u].y, f0 + 1); take(v[u].z, f0 + 2); take(v[u].w, f0 + 3);
             }
         }
-        acc += (double)(((fs[0] + fs[1]) + (fs[2] + fs[3])) + ((fs[4] + fs[5]) + (fs[6] + fs[7])));
-    }
+        acc += (double)fs;
 #pragma unroll
-    for (int o = 16; o; o >>= 1) {
-        ProfileBest u = {__shfl_xor_sync(0xffffffffu, up.v, o), __shfl_xor_sync(0xffffffffu, up.k, o)};
-        ProfileBest d = {__shfl_xor_sync(0xffffffffu, dn.v, o), __shfl_xor_sync(0xffffffffu, dn.k, o)};
-        up = better(up, u); dn = better(dn, d);
-        acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        for (int u = 0; u < U; u++) v[u] = nx[u];
     }
+    auto warp_best = [&]() {
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            ProfileBest u = {__shfl_xor_sync(0xffffffffu, up.v, o), __shfl_xor_sync(0xffffffffu, up.k, o)};
+            ProfileBest d = {__shfl_xor_sync(0xffffffffu, dn.v, o), __shfl_xor_sync(0xffffffffu, dn.k, o)};
+            up = better(up, u); dn = better(dn, d);
+            acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        }
+    };
+    warp_best();
     if (lane == 0) { sb[0][warp] = up; sb[1][warp] = dn; ssum[warp] = acc; }
     __syncthreads();
-    if (tid == 0) {
-        for (int w = 1; w < 8; w++) { up = better(up, sb[0][w]); dn = better(dn, sb[1][w]); acc += ssum[w]; }
-        sk[0] = up.k; sk[1] = dn.k;
-        stotal = acc;
-        k_up[blockIdx.x] = up.k; k_dn[blockIdx.x] = dn.k;
-        p_up[blockIdx.x] = up.v / (float)n_ipp;
-        p_dn[blockIdx.x] = dn.v / (float)n_ipp;
-    }
-    __syncthreads();
     // the bins within `guard` of either line (each once, inside the searched range): at most 2 (2 guard + 1)
-    const int ku = sk[0], kd = sk[1];
     const int g = guard < N ? guard : N, wlen = 2 * g + 1;
+    const bool one_warp = 2 * wlen <= 32;                               // the usual case: warp 0 finishes the row alone
+    if (warp == 0) {
+        up = lane < W ? sb[0][lane] : none; dn = lane < W ? sb[1][lane] : none;
+        acc = lane < W ? ssum[lane] : 0.0;
+        warp_best();                                                    // every lane of warp 0 now holds the row's results
+        if (lane == 0) {
+            k_up[blockIdx.x] = up.k; k_dn[blockIdx.x] = dn.k;
+            p_up[blockIdx.x] = up.v / (float)n_ipp;
+            p_dn[blockIdx.x] = dn.v / (float)n_ipp;
+            if (!one_warp) { sk[0] = up.k; sk[1] = dn.k; stotal = acc; }
+        }
+    } else if (one_warp) {
+        return;
+    }
+    if (!one_warp) __syncthreads();
+    const int ku = one_warp ? up.k : sk[0], kd = one_warp ? dn.k : sk[1];
     double ex = 0.0;
     int nex = 0;
-    for (int j = tid; j < 2 * wlen; j += 256) {
+    for (int j = one_warp ? lane : tid; j < 2 * wlen; j += one_warp ? 32 : T) {
         const bool second = j >= wlen;
         const int f = (second ? kd : ku) - g + (second ? j - wlen : j);
         const int du = f > ku ? f - ku : ku - f;
@@ -342,12 +357,16 @@ __global__ void __launch_bounds__(256) profile_kernel(const float *__restrict__ 
         ex += __shfl_xor_sync(0xffffffffu, ex, o);
         nex += __shfl_xor_sync(0xffffffffu, nex, o);
     }
-    if (lane == 0) { ssum[warp] = ex; scnt[warp] = nex; }
-    __syncthreads();
+    if (!one_warp) {
+        if (lane == 0) { ssum[warp] = ex; scnt[warp] = nex; }
+        __syncthreads();
+        if (tid != 0) return;
+        for (int w = 1; w < W; w++) { ex += ssum[w]; nex += scnt[w]; }
+        acc = stotal;
+    }
     if (tid == 0) {
-        for (int w = 1; w < 8; w++) { ex += ssum[w]; nex += scnt[w]; }
         const int cnt = (hi - lo) - nex;                               // hi - lo + 1 searched bins less N/2
-        noise[blockIdx.x] = cnt > 0 ? (float)((stotal - ex) / (double)cnt / (double)n_ipp) : 0.f;
+        noise[blockIdx.x] = cnt > 0 ? (float)((acc - ex) / (double)cnt / (double)n_ipp) : 0.f;
     }
 }
 
