@@ -381,10 +381,16 @@ def main():
                     help="workloads whose code repeats every IPP (cfg4's chirp): pass the one code (PLSPEC_OPT_SHARED_CODE)")
     ap.add_argument("--n-ipp", type=int, default=0, help="experiments: override the workload's IPP count")
     ap.add_argument("--n-ranges", type=int, default=0, help="experiments: override the workload's gate count")
+    ap.add_argument("--input", default="", choices=["", "sc16", "complex64"],
+                    help="experiments: override the workload's voltage dtype")
     args = ap.parse_args()
     w = synth.CONFIGS[args.workload]
     if args.n_ipp or args.n_ranges:
         w = synth.scaled(w, n_ranges=args.n_ranges or None, n_ipp=args.n_ipp or None, ipp_len=w.ipp_len)
+    if args.input:
+        from dataclasses import replace
+        w = replace(w, dtype=synth.SC16 if args.input == "sc16" else synth.CF32,
+                    sigma=1000.0 if args.input == "sc16" and w.dtype != synth.SC16 else w.sigma)
     if args.impl == "reference":
         return run_reference(args, w)
     if args.probe_mem:

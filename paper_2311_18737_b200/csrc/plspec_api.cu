@@ -146,8 +146,9 @@ const void *fused_ptr(int dt) {
 }
 // the outer radix Q > 1 only occurs with the largest inner size (Nk = 16384, RA = 16).  `prefetch`: the direct-load
 // kernel at Nk = 16384 may fetch the whole next window ahead of time (only safe when code_len == N)
-const void *fused_lookup(int RA, int Q, int dt, bool st, bool prefetch) {
+const void *fused_lookup(int RA, int Q, int dt, bool st, bool prefetch, bool early_decode) {
     if (Q == 1) {
+        if (early_decode) return (const void *)fused_kernel<16, 1, DT_SC16, true, true, 0, DT_CF32, false, true>;
         if (RA == 16 && !st && !prefetch) return fused_ptr<16, 1, false, false>(dt);
         switch (RA) {
             case 1:  return st ? fused_ptr<1, 1, true>(dt) : fused_ptr<1, 1, false>(dt);
@@ -183,8 +184,13 @@ int select_kernel(plspec_ctx *h) {
         // the stage only adds shared-memory traffic), 2 = wherever it fits, 0 = never
         h->staged = h->opt_stage && h->Q == 1 && run + 32 <= (long long)kStageMaxBytes &&
                     (h->gates_per_cta > 1 || h->opt_stage == 2);
+        // early decode (plspec_fused.cuh, ED): sc16 windows of 16384 with a full-length code go through the stage
+        // after all, because the next window is then decoded from it inside the last butterfly stage of the current one
+        const bool early = h->opt_stage == 1 && h->RA == 16 && h->Q == 1 && dt == DT_SC16 && h->L == h->N &&
+                           run + 32 <= (long long)kStageMaxBytes;
+        if (early) h->staged = true;
         if (h->staged) h->smem = (size_t)kStageOff + (size_t)((run + 15) / 16 * 16 + 16);
-        h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged, h->L == h->N);
+        h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged, h->L == h->N, early);
         h->split = h->opt_split == 1 && h->Q > 1;
         h->ring_mode = h->opt_split == 2 && h->Q > 1;
         if (h->ring_mode) {

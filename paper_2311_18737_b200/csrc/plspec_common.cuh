@@ -38,6 +38,8 @@ struct KParams {
     int ring_ahead;         // steps a slice is produced ahead of its use
     int c_pitch;            // samples between successive code rows (0: one code for every IPP)
     int ring_stage;         // 1: the producers' inputs go through shared memory (bulk copies one step ahead)
+    int zero;               // always 0, but only known at run time: an operand the assembler cannot fold, used to pin the
+                            // order of independent instruction groups (plspec_fused.cuh, early decode)
 };
 
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }

@@ -24,6 +24,7 @@
 //
 // Shared memory: 16 regions (one per B warp) of 16*65 8-byte slots + the B1->B2 twiddle table.
 //   A -> B1 :  slot (a'*2 + plane)*32 + b        holds (y[32(2a')+b], y[32(2a'+1)+b]).plane      (STS.64 / LDS.64)
+//              RA = 16: 16-byte slot a'*32 + b   holds both planes of that pair                    (STS.128 / LDS.128)
 //   B1 -> B2:  slot  bb*65 + plane*32 + c        holds (z[c][bb], z[c][bb+16]).plane             (STS.32 / LDS.64)
 // Both are free of bank conflicts (the 65 pitch spreads the 4-byte transposed stores over all banks).
 //
@@ -454,8 +455,17 @@ __device__ __noinline__ void ring_produce_lean_fn(const KParams *P, int sp, int 
 // The decoded windows never reach DRAM: the scratch round trip of the old split path (2 x 21 GB at cfg 4) is gone.
 // IDC = true: identity code -- the windows are decoded already (step 2 of the scratch path for N > 16384): pass A
 // takes the prefetched complex64 words as they are (no code words, no sign flips).
-template <int RA, int Q, int DT, bool ST, bool PFE = true, int RQ = 0, int VDT = DT_CF32, bool IDC = false>
+// ED = true: EARLY DECODE (ST, RA = 16, Q = 1, sc16).  With one gate per CTA the stage does not save loads, but it puts
+// the next window's raw samples a shared-memory load away while the current window is still in pass B2 -- and the last
+// butterfly stage retires eight registers per step.  So for +-1 codes the next window is decoded right there: after
+// step k of the last stage the two sample pairs whose registers just died are read from the stage, converted and
+// sign-flipped (PRMT / LOP3 / IADD3: the half-rate ALU pipe) between the multiply-adds of step k + 1 (FMA pipe), and
+// the window starts with its DFT over t_hi.  Without this every warp of the SM decodes at the same time at the top
+// of a window, the ALU pipe saturates and the FMA pipe idles (removing 64 of the 167 decode instructions, as an
+// experiment, made cfg 3 7.6 % faster).  The copy of window i + 2 starts when all 16 warps have decoded window i + 1.
+template <int RA, int Q, int DT, bool ST, bool PFE = true, int RQ = 0, int VDT = DT_CF32, bool IDC = false, bool ED = false>
 __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_constant__ KParams P) {
+    static_assert(!ED || (ST && RA == 16 && Q == 1 && DT == DT_SC16 && RQ == 0 && !IDC), "early decode: staged sc16 windows of 16384");
     static_assert(!ST || Q == 1, "the staged variant holds one whole window run in shared memory");
     static_assert(RQ == 0 || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && PFE), "ring mode: 16384-point complex64 windows");
     static_assert(!IDC || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && PFE && RQ == 0), "identity code: prefetching complex64 variant");
@@ -464,6 +474,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     constexpr int G = 16 / RA;             // gates per CTA
     constexpr int LOGRA = ilog2(RA);
     constexpr int FG = RA == 16 ? 4 : 1;   // regions per "full" mbarrier (measured: 4 at RA = 16, 1 below)
+    // A -> B1 exchange in 128-bit accesses, slot (a' * 32 + b) of 16 bytes = (y.re pair, y.im pair): half the shared-memory
+    // instructions for the same wavefronts.  Measured: cfg 3 5.974 -> 5.923 ms, paper workload 12.63 -> 12.38 ms; at
+    // RA = 8 and 4 the quad-aligned registers cost spills (cfg 5 28.2 -> 28.5 ms), so those keep the 64-bit layout.
+    constexpr bool X128 = RA == 16;
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = warp / RA, wa = warp % RA;       // pass A: warp `wa` of gate g;  pass B: (gate g, f_hi = wa)
@@ -671,6 +685,50 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
         }
     }
 
+    // The walk over this CTA's work items, compiled once, or twice in the ED kernel: EDM = early decode in effect
+    // (+-1 codes), where the decoded next window is carried from the tail of one window to the top of the next --
+    // 64 registers that must not exist on the general-code path.
+    auto run = [&](auto edm_) {
+    constexpr bool EDM = decltype(edm_)::value;
+    float2 nxr[EDM ? 16 : 1], nxi[EDM ? 16 : 1];
+    auto ed_src = [&](int t, int pp, uint32_t &cw) {   // this thread's first sample of (tile t, IPP pp) in the stage; its code word
+        const int rr = t < P.R ? t : P.R - 1;          // G == 1: tile = gate group = gate
+        const uintptr_t a = reinterpret_cast<uintptr_t>(P.V) +
+                            (uintptr_t)(((long long)pp * P.v_pitch + (long long)P.r0 + (long long)t * P.stride) * ESZ);
+        cw = __ldg(P.Cbits + (long long)pp * 512 + wa * 32 + lane);
+        return reinterpret_cast<const uint32_t *>(stage) + (int)((a & 15) / ESZ) + (rr - t) * P.stride + 64 * wa + lane;
+    };
+    auto ed_dec = [&](auto th_, const uint32_t *src, uint32_t cw) {   // samples th 1024 + t_lo (+ 32) -> nxr / nxi[th]
+        constexpr int th = decltype(th_)::value;
+        if constexpr (EDM)
+            sc16_pair_to_f32(src[th * 1024], src[th * 1024 + 32], bit_mask<2 * th>(cw), bit_mask<2 * th + 1>(cw), nxr[th], nxi[th]);
+    };
+    auto ed_arrive = [&](bool issue, int t, int pp) {  // this warp is done with the stage; the 16th warp starts the next copy
+        __syncwarp();
+        if (lane == 0) {
+            __threadfence_block();
+            const int old = atomicAdd(cnt, 1);
+            if (old == arrivals_target && issue) {
+                __threadfence_block();
+                fence_proxy_async();
+                stage_issue(t, pp);
+            }
+        }
+        arrivals_target += 16;
+    };
+    if constexpr (EDM) {
+        {                                              // the first window: nothing to hide it under
+            uint32_t cw0;
+            const uint32_t *s0 = ed_src(tile0, p0, cw0);
+            mbar_wait(mbar, parity);
+            parity ^= 1u;
+            sfor<0, 16>([&](auto th_) { ed_dec(th_, s0, cw0); });
+            int p1 = p0 + 1, t1 = tile0;
+            if (p1 == P.n_ipp) { p1 = 0; t1++; }
+            ed_arrive(i1 - i0 >= 2, t1, p1);
+        }
+    }
+
     int left = (int)(i1 - i0);                     // items still to do, this one included
     int p_lo = p0;
     // ring mode: a "tile" is a run of at most kRingFlushEvery pulses of one round -- two-level summation: fp32 sums of
@@ -721,10 +779,12 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
         VSrc vs;
         vs.V = P.V; vs.voff = voff; vs.stage = stage; vs.sbase = 0;
         if constexpr (ST) {
-            const uintptr_t a = reinterpret_cast<uintptr_t>(P.V) + (uintptr_t)(((long long)p * P.v_pitch + run_off) * ESZ);
-            vs.sbase = (int)((a & 15) / ESZ) + (r_ld - gg * G) * P.stride;
-            mbar_wait(mbar, parity);
-            parity ^= 1u;
+            if constexpr (!EDM) {
+                const uintptr_t a = reinterpret_cast<uintptr_t>(P.V) + (uintptr_t)(((long long)p * P.v_pitch + run_off) * ESZ);
+                vs.sbase = (int)((a & 15) / ESZ) + (r_ld - gg * G) * P.stride;
+                mbar_wait(mbar, parity);
+                parity ^= 1u;
+            }
         }
         float2 xr[16], xi[16];
         // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
@@ -734,6 +794,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                 xr[th] = make_float2(__uint_as_float(raw[4 * th]), __uint_as_float(raw[4 * th + 2]));
                 xi[th] = make_float2(__uint_as_float(raw[4 * th + 1]), __uint_as_float(raw[4 * th + 3]));
             });
+        } else if constexpr (EDM) {                                  // decoded in the tail of the previous window
+#pragma unroll
+            for (int j = 0; j < 16; j++) { xr[j] = nxr[j]; xi[j] = nxi[j]; }
         } else if (PF && bpsk) {
             if constexpr (PF) {
                 sfor<0, RA>([&](auto th_) {
@@ -794,26 +857,21 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
         if constexpr (RQ > 0) ring_arrive(1, rs);                   // this warp's loads of the slot have all returned
         if constexpr (ST) {
             // this warp has consumed its samples of IPP p; the last of the 16 warps starts the copy of IPP p + 1
-            __syncwarp();
-            if (lane == 0) {
-                __threadfence_block();
-                const int old = atomicAdd(cnt, 1);
-                if (old == arrivals_target && has_next) {
-                    __threadfence_block();
-                    fence_proxy_async();
-                    stage_issue(tile_next, p_next);
-                }
-            }
-            arrivals_target += 16;
+            if constexpr (!EDM) ed_arrive(has_next, tile_next, p_next);
         }
         if constexpr (RA == 1) __syncwarp();
         else mbar_wait(free_base, free_parity);                          // every owner has read the previous window
         auto store_y = [&](auto jj_, auto f_, float2 yr, float2 yi) {   // y_{f}[t_lo] -> region of pass-B warp (g, f)
             constexpr int jj = decltype(jj_)::value, f = decltype(f_)::value;
             const int ap = wa + RA * jj;
-            float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
-            dst[0] = yr;
-            dst[32] = yi;
+            if constexpr (X128) {
+                float4 *dst = reinterpret_cast<float4 *>(gate_regions + f * kRegionBytes) + ap * 32 + lane;
+                *dst = make_float4(yr.x, yr.y, yi.x, yi.y);
+            } else {
+                float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
+                dst[0] = yr;
+                dst[32] = yi;
+            }
             if constexpr (RA > 1 && jj == NJ - 1 && (f % FG == FG - 1 || f == RA - 1)) {   // last store into the regions of group f / FG
                 __syncwarp();
                 if (lane == 0) mbar_arrive(full_base + 8 * (f / FG));
@@ -859,11 +917,21 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
 
         // ---- pass B1: lane = b; decimation-in-time radix-32 over a; .x = even a, .y = odd a
         {
-            const float2 *src = reinterpret_cast<const float2 *>(region) + lane;
+            if constexpr (X128) {
+                const float4 *src = reinterpret_cast<const float4 *>(region) + lane;
 #pragma unroll
-            for (int ap = 0; ap < 16; ap++) {
-                xr[ap] = src[(ap * 2) * 32];
-                xi[ap] = src[(ap * 2 + 1) * 32];
+                for (int ap = 0; ap < 16; ap++) {
+                    const float4 v = src[ap * 32];
+                    xr[ap] = make_float2(v.x, v.y);
+                    xi[ap] = make_float2(v.z, v.w);
+                }
+            } else {
+                const float2 *src = reinterpret_cast<const float2 *>(region) + lane;
+#pragma unroll
+                for (int ap = 0; ap < 16; ap++) {
+                    xr[ap] = src[(ap * 2) * 32];
+                    xi[ap] = src[(ap * 2 + 1) * 32];
+                }
             }
         }
         __syncwarp();
@@ -899,23 +967,49 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             }
         }
         // ---- pass B2: lane = c; decimation-in-frequency radix-32 over b; .x = b, .y = b + 16
-        {
-            const float2 *src = reinterpret_cast<const float2 *>(region) + lane;
+        auto b2_front = [&]() {
+            {
+                const float2 *src = reinterpret_cast<const float2 *>(region) + lane;
 #pragma unroll
-            for (int bb = 0; bb < 16; bb++) {
-                xr[bb] = src[bb * 65];
-                xi[bb] = src[bb * 65 + 32];
+                for (int bb = 0; bb < 16; bb++) {
+                    xr[bb] = src[bb * 65];
+                    xi[bb] = src[bb * 65 + 32];
+                }
+            }
+            if constexpr (RA > 1) {                                  // this warp's region may be overwritten again
+                __syncwarp();
+                if (lane == 0) mbar_arrive(free_base);
+            }
+            sfor<0, 16>([&](auto b_) {
+                constexpr int bb = decltype(b_)::value;
+                bfly_dif_halves<bb>(xr[bb], xi[bb]);                 // (.x, .y) -> (even e, odd e) inputs
+            });
+            dft_packed16_head(xr, xi);
+        };
+        if constexpr (EDM) {
+            if (has_next) {                                      // pass B2 with the next window's decode in between
+                uint32_t cwn;
+                const uint32_t *sn = ed_src(tile_next, p_next, cwn);
+                mbar_wait(mbar, parity);                         // its copy started a window ago
+                parity ^= 1u;
+                b2_front();                                      // same basic block as the decode below: the assembler may
+                                                                 // start it as early as it finds registers
+                sfor<0, 8>([&](auto k_) {
+                    constexpr int k = decltype(k_)::value;
+                    constexpr int ia = brev<4>(k), ib = brev<4>(k + 8);
+                    bfly_power<2 * k>(xr[ia], xi[ia], xr[ib], xi[ib], accS[k], accC[k]);
+                    // the loads of this step hang on its last multiply-add through a zero the assembler cannot see:
+                    // otherwise it moves all 32 loads (and their conversions) to the front, where no register is free
+                    ed_dec(std::integral_constant<int, ia>{}, sn, cwn);      // into the registers that just died
+                    ed_dec(std::integral_constant<int, ib>{}, sn, cwn);
+                });
+                int p2 = p_next + 1, t2 = tile_next;
+                if (p2 == P.n_ipp) { p2 = 0; t2++; }
+                ed_arrive((p_hi - 1 - p) + left >= 2, t2, p2);
+                continue;
             }
         }
-        if constexpr (RA > 1) {                                  // this warp's region may be overwritten again
-            __syncwarp();
-            if (lane == 0) mbar_arrive(free_base);
-        }
-        sfor<0, 16>([&](auto b_) {
-            constexpr int bb = decltype(b_)::value;
-            bfly_dif_halves<bb>(xr[bb], xi[bb]);                 // (.x, .y) -> (even e, odd e) inputs
-        });
-        dft_packed16_head(xr, xi);
+        b2_front();
         const uint32_t *pf_next = nullptr;
         if constexpr (RQ > 0) {
             if (has_next) ring_wait(0, rs + 1);                  // the next window is in the ring (it has been for a while)
@@ -939,6 +1033,12 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                 }
             }
         });
+        if constexpr (EDM) {
+            // only the CTA's last window comes this way, but the compiler cannot know: without a definition here the
+            // 64 carried registers would count as live through the whole loop body on this path, and be spilled
+#pragma unroll
+            for (int j = 0; j < 16; j++) nxr[j] = nxi[j] = make_float2(0.f, 0.f);
+        }
     }
     // ---- flush: S_dev[r][q][f_hi = wa][e][c = lane]; other CTAs may hold the rest of this tile's IPPs
     if (r < Rv) {
@@ -957,6 +1057,13 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             atomicAdd(Srow + (e + 1) * 32, acc[j].y);
         });
     }
+    }
+    };   // run
+    if constexpr (ED) {
+        if (bpsk) run(std::true_type{});
+        else run(std::false_type{});
+    } else {
+        run(std::false_type{});
     }
 
     tmem_fence_before_sync();
