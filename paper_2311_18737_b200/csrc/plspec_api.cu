@@ -139,16 +139,24 @@ int device_sm_count() {
     return n;
 }
 
-template <int RA, int Q, bool ST, bool PFE = true>
+template <int RA, int Q, bool ST, bool PFE = true, bool ED = false>
 const void *fused_ptr(int dt) {
-    return dt == DT_CF32 ? (const void *)fused_kernel<RA, Q, DT_CF32, ST, PFE>
-                         : (const void *)fused_kernel<RA, Q, DT_SC16, ST, PFE>;
+    return dt == DT_CF32 ? (const void *)fused_kernel<RA, Q, DT_CF32, ST, PFE, 0, DT_CF32, false, ED>
+                         : (const void *)fused_kernel<RA, Q, DT_SC16, ST, PFE, 0, DT_CF32, false, ED>;
 }
 // the outer radix Q > 1 only occurs with the largest inner size (Nk = 16384, RA = 16).  `prefetch`: the direct-load
 // kernel at Nk = 16384 may fetch the whole next window ahead of time (only safe when code_len == N)
 const void *fused_lookup(int RA, int Q, int dt, bool st, bool prefetch, bool early_decode) {
     if (Q == 1) {
-        if (early_decode) return (const void *)fused_kernel<16, 1, DT_SC16, true, true, 0, DT_CF32, false, true>;
+        if (early_decode && st) {
+            switch (RA) {
+                case 1:  return fused_ptr<1, 1, true, true, true>(dt);
+                case 2:  return fused_ptr<2, 1, true, true, true>(dt);
+                case 4:  return fused_ptr<4, 1, true, true, true>(dt);
+                case 8:  return fused_ptr<8, 1, true, true, true>(dt);
+                case 16: return fused_ptr<16, 1, true, true, true>(dt);
+            }
+        }
         if (RA == 16 && !st && !prefetch) return fused_ptr<16, 1, false, false>(dt);
         switch (RA) {
             case 1:  return st ? fused_ptr<1, 1, true>(dt) : fused_ptr<1, 1, false>(dt);
@@ -184,11 +192,12 @@ int select_kernel(plspec_ctx *h) {
         // the stage only adds shared-memory traffic), 2 = wherever it fits, 0 = never
         h->staged = h->opt_stage && h->Q == 1 && run + 32 <= (long long)kStageMaxBytes &&
                     (h->gates_per_cta > 1 || h->opt_stage == 2);
-        // early decode (plspec_fused.cuh, ED): sc16 windows of 16384 with a full-length code go through the stage
-        // after all, because the next window is then decoded from it inside the last butterfly stage of the current one
-        const bool early = h->opt_stage == 1 && h->RA == 16 && h->Q == 1 && dt == DT_SC16 && h->L == h->N &&
-                           run + 32 <= (long long)kStageMaxBytes;
-        if (early) h->staged = true;
+        // early decode (plspec_fused.cuh, ED; the default, opt_stage == 1): with a full-length code the next window is
+        // decoded from the stage inside the last butterfly stage of the current one; sc16 windows of 16384 go through
+        // the stage for that reason alone
+        if (h->opt_stage == 1 && h->RA == 16 && h->Q == 1 && dt == DT_SC16 && h->L == h->N && run + 32 <= (long long)kStageMaxBytes)
+            h->staged = true;
+        const bool early = h->opt_stage == 1 && h->staged && h->L == h->N;
         if (h->staged) h->smem = (size_t)kStageOff + (size_t)((run + 15) / 16 * 16 + 16);
         h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged, h->L == h->N, early);
         h->split = h->opt_split == 1 && h->Q > 1;

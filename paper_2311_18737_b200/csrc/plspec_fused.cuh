@@ -455,17 +455,19 @@ __device__ __noinline__ void ring_produce_lean_fn(const KParams *P, int sp, int 
 // The decoded windows never reach DRAM: the scratch round trip of the old split path (2 x 21 GB at cfg 4) is gone.
 // IDC = true: identity code -- the windows are decoded already (step 2 of the scratch path for N > 16384): pass A
 // takes the prefetched complex64 words as they are (no code words, no sign flips).
-// ED = true: EARLY DECODE (ST, RA = 16, Q = 1, sc16).  With one gate per CTA the stage does not save loads, but it puts
-// the next window's raw samples a shared-memory load away while the current window is still in pass B2 -- and the last
-// butterfly stage retires eight registers per step.  So for +-1 codes the next window is decoded right there: after
-// step k of the last stage the two sample pairs whose registers just died are read from the stage, converted and
-// sign-flipped (PRMT / LOP3 / IADD3: the half-rate ALU pipe) between the multiply-adds of step k + 1 (FMA pipe), and
-// the window starts with its DFT over t_hi.  Without this every warp of the SM decodes at the same time at the top
-// of a window, the ALU pipe saturates and the FMA pipe idles (removing 64 of the 167 decode instructions, as an
-// experiment, made cfg 3 7.6 % faster).  The copy of window i + 2 starts when all 16 warps have decoded window i + 1.
+// ED = true: EARLY DECODE (staged variants, Q = 1; +-1 codes).  The stage puts the next window's raw samples a
+// shared-memory load away while the current window is still in pass B2, and the last butterfly stage retires eight
+// registers per step.  So the next window is decoded right there: after step k of the last stage the two sample
+// pairs whose registers just died are read from the stage, converted and sign-flipped (PRMT / LOP3 / IADD3: the
+// half-rate ALU pipe) between the multiply-adds of the following steps (FMA pipe), and the window starts with its DFT
+// over t_hi.  Without this every warp of the SM decodes at the same time at the top of a window: the ALU pipe saturates
+// and the FMA pipe idles (removing 64 of the 167 decode instructions, as an experiment, made cfg 3 7.6 % faster).  The
+// copy of window i + 2 starts when all 16 warps have decoded window i + 1.  At RA = 16 (one gate per CTA) the stage
+// saves no loads and exists for this alone (sc16 only: a complex64 window of 16384 does not fit beside the exchange).
+// Measured: cfg 3 5.93 -> 5.81 ms (staged without early decode: 6.10), cfg 2 0.350 -> 0.346 ms, cfg 5 unchanged.
 template <int RA, int Q, int DT, bool ST, bool PFE = true, int RQ = 0, int VDT = DT_CF32, bool IDC = false, bool ED = false>
 __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_constant__ KParams P) {
-    static_assert(!ED || (ST && RA == 16 && Q == 1 && DT == DT_SC16 && RQ == 0 && !IDC), "early decode: staged sc16 windows of 16384");
+    static_assert(!ED || (ST && Q == 1 && RQ == 0 && !IDC), "early decode: staged windows");
     static_assert(!ST || Q == 1, "the staged variant holds one whole window run in shared memory");
     static_assert(RQ == 0 || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && PFE), "ring mode: 16384-point complex64 windows");
     static_assert(!IDC || (RA == 16 && Q == 1 && DT == DT_CF32 && !ST && PFE && RQ == 0), "identity code: prefetching complex64 variant");
@@ -691,17 +693,31 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     auto run = [&](auto edm_) {
     constexpr bool EDM = decltype(edm_)::value;
     float2 nxr[EDM ? 16 : 1], nxi[EDM ? 16 : 1];
-    auto ed_src = [&](int t, int pp, uint32_t &cw) {   // this thread's first sample of (tile t, IPP pp) in the stage; its code word
-        const int rr = t < P.R ? t : P.R - 1;          // G == 1: tile = gate group = gate
+    // this thread's sample 0 of its gate's window of (tile t, IPP pp) in the stage (+ lane); its code words
+    auto ed_src = [&](int t, int pp, uint32_t *cw) {
+        const int rr = t * G + g < P.R ? t * G + g : P.R - 1;          // Q == 1: tile = gate group
         const uintptr_t a = reinterpret_cast<uintptr_t>(P.V) +
-                            (uintptr_t)(((long long)pp * P.v_pitch + (long long)P.r0 + (long long)t * P.stride) * ESZ);
-        cw = __ldg(P.Cbits + (long long)pp * 512 + wa * 32 + lane);
-        return reinterpret_cast<const uint32_t *>(stage) + (int)((a & 15) / ESZ) + (rr - t) * P.stride + 64 * wa + lane;
+                            (uintptr_t)(((long long)pp * P.v_pitch + (long long)P.r0 + (long long)(t * G) * P.stride) * ESZ);
+#pragma unroll
+        for (int jj = 0; jj < NJ; jj++) cw[jj] = __ldg(P.Cbits + (long long)pp * 512 + (wa + RA * jj) * 32 + lane);
+        return stage + ((long long)((a & 15) / ESZ) + (long long)(rr - t * G) * P.stride + lane) * ESZ;
     };
-    auto ed_dec = [&](auto th_, const uint32_t *src, uint32_t cw) {   // samples th 1024 + t_lo (+ 32) -> nxr / nxi[th]
-        constexpr int th = decltype(th_)::value;
-        if constexpr (EDM)
-            sc16_pair_to_f32(src[th * 1024], src[th * 1024 + 32], bit_mask<2 * th>(cw), bit_mask<2 * th + 1>(cw), nxr[th], nxi[th]);
+    // element e = jj RA + th of the thread: samples th 1024 + 64 (wa + RA jj) + lane (+ 32) -> nxr / nxi[e]
+    auto ed_dec = [&](auto e_, const unsigned char *src, const uint32_t *cw) {
+        constexpr int e = decltype(e_)::value, jj = e / RA, th = e % RA;
+        if constexpr (EDM) {
+            const int t0 = th * 1024 + 64 * (wa + RA * jj);
+            const uint32_t m0 = bit_mask<2 * th>(cw[jj]), m1 = bit_mask<2 * th + 1>(cw[jj]);
+            if constexpr (DT == DT_SC16) {
+                const uint32_t *w = reinterpret_cast<const uint32_t *>(src) + t0;
+                sc16_pair_to_f32(w[0], w[32], m0, m1, nxr[e], nxi[e]);
+            } else {
+                const uint2 *w = reinterpret_cast<const uint2 *>(src) + t0;
+                const uint2 z0 = w[0], z1 = w[32];
+                nxr[e] = make_float2(__uint_as_float(z0.x ^ (m0 & 0x80000000u)), __uint_as_float(z1.x ^ (m1 & 0x80000000u)));
+                nxi[e] = make_float2(__uint_as_float(z0.y ^ (m0 & 0x80000000u)), __uint_as_float(z1.y ^ (m1 & 0x80000000u)));
+            }
+        }
     };
     auto ed_arrive = [&](bool issue, int t, int pp) {  // this warp is done with the stage; the 16th warp starts the next copy
         __syncwarp();
@@ -718,8 +734,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     };
     if constexpr (EDM) {
         {                                              // the first window: nothing to hide it under
-            uint32_t cw0;
-            const uint32_t *s0 = ed_src(tile0, p0, cw0);
+            uint32_t cw0[NJ];
+            const unsigned char *s0 = ed_src(tile0, p0, cw0);
             mbar_wait(mbar, parity);
             parity ^= 1u;
             sfor<0, 16>([&](auto th_) { ed_dec(th_, s0, cw0); });
@@ -988,8 +1004,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
         };
         if constexpr (EDM) {
             if (has_next) {                                      // pass B2 with the next window's decode in between
-                uint32_t cwn;
-                const uint32_t *sn = ed_src(tile_next, p_next, cwn);
+                uint32_t cwn[NJ];
+                const unsigned char *sn = ed_src(tile_next, p_next, cwn);
                 mbar_wait(mbar, parity);                         // its copy started a window ago
                 parity ^= 1u;
                 b2_front();                                      // same basic block as the decode below: the assembler may
