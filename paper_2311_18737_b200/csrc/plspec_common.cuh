@@ -38,8 +38,6 @@ struct KParams {
     int ring_ahead;         // steps a slice is produced ahead of its use
     int c_pitch;            // samples between successive code rows (0: one code for every IPP)
     int ring_stage;         // 1: the producers' inputs go through shared memory (bulk copies one step ahead)
-    int zero;               // always 0, but only known at run time: an operand the assembler cannot fold, used to pin the
-                            // order of independent instruction groups (plspec_fused.cuh, early decode)
 };
 
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
@@ -88,6 +86,19 @@ __device__ __forceinline__ void sc16_pair_to_f32(uint32_t w0, uint32_t w1, uint3
     const float2 k = make_float2(__uint_as_float(0xCB008000u + m0), __uint_as_float(0xCB008000u + m1));   // -(2^23 + 32768) [+ 1]
     re = __fadd2_rn(fr, k);
     im = __fadd2_rn(fi, k);
+}
+
+// The same conversion through the conversion unit (I2F.S16 with a half-word operand; 16 lanes per clock and SM, its
+// own pipe) and one packed multiply by +-1: three ALU-pipe instructions per sample fewer than the form above, at two
+// I2F per sample.  Used for every other sample pair where the ALU pipe is the bottleneck (early decode, plspec_fused.cuh).
+// Exact like the other: the conversion is exact and so is the product with +-1 (a zero sample may come out as -0).
+__device__ __forceinline__ void sc16_pair_to_f32_xu(uint32_t w0, uint32_t w1, uint32_t m0, uint32_t m1, float2 &re, float2 &im) {
+    float r0, i0, r1, i1;
+    asm("{\n.reg .b16 lo, hi;\nmov.b32 {lo, hi}, %2;\ncvt.rn.f32.s16 %0, lo;\ncvt.rn.f32.s16 %1, hi;\n}" : "=f"(r0), "=f"(i0) : "r"(w0));
+    asm("{\n.reg .b16 lo, hi;\nmov.b32 {lo, hi}, %2;\ncvt.rn.f32.s16 %0, lo;\ncvt.rn.f32.s16 %1, hi;\n}" : "=f"(r1), "=f"(i1) : "r"(w1));
+    const float2 s = make_float2(__uint_as_float((m0 & 0x80000000u) | 0x3F800000u), __uint_as_float((m1 & 0x80000000u) | 0x3F800000u));
+    re = __fmul2_rn(make_float2(r0, r1), s);
+    im = __fmul2_rn(make_float2(i0, i1), s);
 }
 
 template <int DT>

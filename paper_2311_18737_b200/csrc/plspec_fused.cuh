@@ -710,7 +710,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             const uint32_t m0 = bit_mask<2 * th>(cw[jj]), m1 = bit_mask<2 * th + 1>(cw[jj]);
             if constexpr (DT == DT_SC16) {
                 const uint32_t *w = reinterpret_cast<const uint32_t *>(src) + t0;
-                sc16_pair_to_f32(w[0], w[32], m0, m1, nxr[e], nxi[e]);
+                // every other pair through the conversion unit: the steps of the last butterfly stage free one even and
+                // one odd element each, so both forms run side by side
+                if constexpr (e & 1) sc16_pair_to_f32_xu(w[0], w[32], m0, m1, nxr[e], nxi[e]);
+                else sc16_pair_to_f32(w[0], w[32], m0, m1, nxr[e], nxi[e]);
             } else {
                 const uint2 *w = reinterpret_cast<const uint2 *>(src) + t0;
                 const uint2 z0 = w[0], z1 = w[32];
@@ -1014,8 +1017,6 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                     constexpr int k = decltype(k_)::value;
                     constexpr int ia = brev<4>(k), ib = brev<4>(k + 8);
                     bfly_power<2 * k>(xr[ia], xi[ia], xr[ib], xi[ib], accS[k], accC[k]);
-                    // the loads of this step hang on its last multiply-add through a zero the assembler cannot see:
-                    // otherwise it moves all 32 loads (and their conversions) to the front, where no register is free
                     ed_dec(std::integral_constant<int, ia>{}, sn, cwn);      // into the registers that just died
                     ed_dec(std::integral_constant<int, ib>{}, sn, cwn);
                 });
