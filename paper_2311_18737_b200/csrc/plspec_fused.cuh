@@ -717,8 +717,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             } else {
                 const uint2 *w = reinterpret_cast<const uint2 *>(src) + t0;
                 const uint2 z0 = w[0], z1 = w[32];
-                nxr[e] = make_float2(__uint_as_float(z0.x ^ (m0 & 0x80000000u)), __uint_as_float(z1.x ^ (m1 & 0x80000000u)));
-                nxi[e] = make_float2(__uint_as_float(z0.y ^ (m0 & 0x80000000u)), __uint_as_float(z1.y ^ (m1 & 0x80000000u)));
+                nxr[e] = make_float2(flip_sign(z0.x, m0), flip_sign(z1.x, m1));
+                nxi[e] = make_float2(flip_sign(z0.y, m0), flip_sign(z1.y, m1));
             }
         }
     };
@@ -824,10 +824,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                     if constexpr (DT == DT_SC16) {
                         sc16_pair_to_f32(raw[2 * th], raw[2 * th + 1], m0, m1, xr[th], xi[th]);
                     } else {                                     // +-1 code: flip the sign bits
-                        xr[th] = make_float2(__uint_as_float(raw[4 * th] ^ (m0 & 0x80000000u)),
-                                             __uint_as_float(raw[4 * th + 2] ^ (m1 & 0x80000000u)));
-                        xi[th] = make_float2(__uint_as_float(raw[4 * th + 1] ^ (m0 & 0x80000000u)),
-                                             __uint_as_float(raw[4 * th + 3] ^ (m1 & 0x80000000u)));
+                        xr[th] = make_float2(flip_sign(raw[4 * th], m0), flip_sign(raw[4 * th + 2], m1));
+                        xi[th] = make_float2(flip_sign(raw[4 * th + 1], m0), flip_sign(raw[4 * th + 3], m1));
                     }
                 });
             }

@@ -105,10 +105,8 @@ __device__ __forceinline__ void load_pair_bpsk(const VSrc &src, uint32_t cw, int
         sc16_pair_to_f32(w0, w1, m0, m1, xr, xi);
     } else {
         const float2 z0 = fetch_voltage<DT, STAGED>(src, t0), z1 = fetch_voltage<DT, STAGED>(src, t1);
-        xr = make_float2(__uint_as_float(__float_as_uint(z0.x) ^ (m0 & 0x80000000u)),
-                         __uint_as_float(__float_as_uint(z1.x) ^ (m1 & 0x80000000u)));
-        xi = make_float2(__uint_as_float(__float_as_uint(z0.y) ^ (m0 & 0x80000000u)),
-                         __uint_as_float(__float_as_uint(z1.y) ^ (m1 & 0x80000000u)));
+        xr = make_float2(flip_sign(__float_as_uint(z0.x), m0), flip_sign(__float_as_uint(z1.x), m1));
+        xi = make_float2(flip_sign(__float_as_uint(z0.y), m0), flip_sign(__float_as_uint(z1.y), m1));
     }
 }
 
