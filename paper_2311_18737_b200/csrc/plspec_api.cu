@@ -195,10 +195,12 @@ int select_kernel(plspec_ctx *h) {
         // early decode (plspec_fused.cuh, ED; the default, opt_stage == 1): with a full-length code the next window is
         // decoded from the stage inside the last butterfly stage of the current one; sc16 windows of 16384 go through
         // the stage for that reason alone
-        if (h->opt_stage == 1 && h->RA == 16 && h->Q == 1 && dt == DT_SC16 && h->L == h->N && run + 32 <= (long long)kStageMaxBytes)
-            h->staged = true;
+        // (that kernel's exchange regions are larger: pass B2 in its decimation-in-time form, kDitExtraBytes)
+        const bool dit = h->opt_stage == 1 && h->RA == 16 && h->Q == 1 && dt == DT_SC16 && h->L == h->N &&
+                         run + 32 <= (long long)kStageMaxBytes - kDitExtraBytes;
+        if (dit) h->staged = true;
         const bool early = h->opt_stage == 1 && h->staged && h->L == h->N;
-        if (h->staged) h->smem = (size_t)kStageOff + (size_t)((run + 15) / 16 * 16 + 16);
+        if (h->staged) h->smem = (size_t)kStageOff + (dit ? (size_t)kDitExtraBytes : 0) + (size_t)((run + 15) / 16 * 16 + 16);
         h->kfunc = fused_lookup(h->RA, h->Q, dt, h->staged, h->L == h->N, early);
         h->split = h->opt_split == 1 && h->Q > 1;
         h->ring_mode = h->opt_split == 2 && h->Q > 1;

@@ -35,7 +35,11 @@
 
 namespace plspec {
 
+// A -> B1: 16 x 32 slots of 16 bytes (8192); B1 -> B2: 16 x 65 slots of 8 bytes (8320), or, where pass B2 is the
+// decimation-in-time form (B2D in the kernel), 64 rows (plane, c) of 32 words at a pitch of 34 (8704)
 constexpr int kRegionBytes = 16 * 65 * 8;                    // 8320
+constexpr int kRegionBytesDit = 64 * 34 * 4;                 // 8704: the kernel whose pass B2 is decimation in time
+constexpr int kDitExtraBytes = 16 * (kRegionBytesDit - kRegionBytes);   // what that kernel needs beyond kStageOff
 constexpr int kFusedSmemBytes = 16 * kRegionBytes;
 // control words: stage mbarrier (8) + warp arrival counter (4) + TMEM base (4) + per region a "free" and a
 // "full" mbarrier
@@ -148,6 +152,33 @@ __host__ __device__ constexpr float pow2w(int K32) {
     if (K32 == 0 || K32 == 8) return 2.0f;
     const double c = cosd32(K32), sn = sind32(K32);
     return (float)(2.0 * (absd(c) >= absd(sn) ? c : sn));
+}
+
+// Last stage of a decimation-in-time radix-32 whose halves sit in one register pair, (.x, .y) = (E, O), fused with
+// |X|^2: X[e] = E + W O, X[e + 16] = E - W O, W = W_32^K32, so |X|^2 = (|E|^2 + |O|^2) +- 2 Re(conj(E) W O) with
+// W O = w (p, q) in the tangent / cotangent form: accS += |E|^2 + |O|^2, accC += E_r p + E_i q; the two spectra values
+// are accS +- 2 w accC at flush time (pow2w).
+template <int K32>
+__device__ __forceinline__ void bfly_power_halves(float2 r, float2 i, float &accS, float &accC) {
+    const float er = r.x, ei = i.x, orr = r.y, oi = i.y;
+    accS = fmaf(er, er, accS); accS = fmaf(ei, ei, accS);
+    accS = fmaf(orr, orr, accS); accS = fmaf(oi, oi, accS);
+    if constexpr (K32 == 0) {
+        accC = fmaf(er, orr, accC); accC = fmaf(ei, oi, accC);
+    } else if constexpr (K32 == 8) {                       // W O = (O_i, -O_r)
+        accC = fmaf(er, oi, accC); accC = fmaf(-ei, orr, accC);
+    } else {
+        constexpr double c = cosd32(K32), sn = sind32(K32);
+        float p, q;
+        if constexpr (absd(c) >= absd(sn)) {
+            constexpr float t = (float)(sn / c);
+            p = fmaf(oi, t, orr); q = fmaf(orr, -t, oi);
+        } else {
+            constexpr float t = (float)(c / sn);
+            p = fmaf(orr, t, oi); q = fmaf(oi, t, -orr);
+        }
+        accC = fmaf(er, p, accC); accC = fmaf(ei, q, accC);
+    }
 }
 
 // the first LOG - 1 stages of dft_packed<16, 0>
@@ -480,6 +511,15 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     // instructions for the same wavefronts.  Measured: cfg 3 5.974 -> 5.923 ms, paper workload 12.63 -> 12.38 ms; at
     // RA = 8 and 4 the quad-aligned registers cost spills (cfg 5 28.2 -> 28.5 ms), so those keep the 64-bit layout.
     constexpr bool X128 = RA == 16;
+    // Pass B2 as a decimation-in-time radix-32 (pairs = even / odd b) whose last stage -- the one across the two halves
+    // of a register pair -- is fused with |X|^2 (bfly_power_halves), instead of the decimation-in-frequency form whose
+    // first stage is across the halves: 420 instead of 448 FMA-pipe cycles per thread and window.  Measured: cfg 3
+    // 5.833 -> 5.784 ms with the early-decode sc16 kernel at RA = 16; the other variants lose (register allocation:
+    // the complex64 prefetch kernel spills 184 bytes, cfg 5 28.14 -> 28.35 ms, cfg 2 0.3429 -> 0.3447 ms), so only
+    // that kernel takes this form.
+    constexpr bool kB2Dit = ED && RA == 16 && DT == DT_SC16;
+    constexpr int RB = kB2Dit ? kRegionBytesDit : kRegionBytes;    // region pitch
+    constexpr int CTL = 16 * RB;                                    // control words behind the regions, then the stage
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = warp / RA, wa = warp % RA;       // pass A: warp `wa` of gate g;  pass B: (gate g, f_hi = wa)
@@ -502,7 +542,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     // ---- twiddles live in tensor memory: every thread re-reads only constants it wrote itself
     //   columns [4 e, 4 e + 4), e = (f - 1) NJ + jj:      pass A -> B1, W_Nk^{t_lo f} for the thread's two t_lo
     //   columns [64 + 4 c', ..):                           B1 -> B2,   W_1024^{b c'}, W_1024^{b (c' + 16)}, b = lane
-    uint32_t *const tm_slot = reinterpret_cast<uint32_t *>(smem + kFusedSmemBytes + 12);
+    uint32_t *const tm_slot = reinterpret_cast<uint32_t *>(smem + CTL + 12);
     if (warp == 0) tmem_alloc_512(smem_u32(tm_slot));
     tmem_fence_before_sync();
     __syncthreads();
@@ -529,13 +569,13 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     pdl_wait();   // everything above (TMEM, twiddles) may overlap the code pre-pass / decode pre-pass before us
     const bool bpsk = IDC || (P.Cbits != nullptr && __ldg(P.not_bpsk) != P.epoch);   // warp-uniform
 
-    unsigned char *const region = smem + warp * kRegionBytes;              // this warp's pass-B region
-    unsigned char *const gate_regions = smem + (g * RA) * kRegionBytes;    // regions of this gate (pass A target)
+    unsigned char *const region = smem + warp * RB;                        // this warp's pass-B region
+    unsigned char *const gate_regions = smem + (g * RA) * RB;              // regions of this gate (pass A target)
 
     // ---- ST: stage control.  mbar counts the bytes of one IPP's copy; cnt counts warps done reading it.
-    const uint32_t mbar = smem_u32(smem + kFusedSmemBytes);
-    int *const cnt = reinterpret_cast<int *>(smem + kFusedSmemBytes + 8);
-    const unsigned char *const stage = smem + kStageOff;
+    const uint32_t mbar = smem_u32(smem + CTL);
+    int *const cnt = reinterpret_cast<int *>(smem + CTL + 8);
+    const unsigned char *const stage = smem + CTL + kStageCtlBytes;
     auto stage_issue = [&](int t, int pp) {                                // one thread: run of tile t, IPP pp
         const int tg = group_of(t);
         const int gates_here = (P.R - tg * G) < G ? (P.R - tg * G) : G;
@@ -556,21 +596,21 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     // free_mbar[gate] (count RA): each owner arrives once it has read its region for the last time in a window
     // (B2 loads done); a pass-A warp waits on it before its first store of the next window (by then the last
     // owner is long past that point, and one probe per window is cheaper than one per region).
-    const uint32_t free_base = smem_u32(smem + kFusedSmemBytes + 16) + 8 * (g * RA);
-    const uint32_t full_base = smem_u32(smem + kFusedSmemBytes + 16 + 16 * 8) + 8 * (g * RA);  // + 8 f
+    const uint32_t free_base = smem_u32(smem + CTL + 16) + 8 * (g * RA);
+    const uint32_t full_base = smem_u32(smem + CTL + 16 + 16 * 8) + 8 * (g * RA);  // + 8 f
     if (tid == 0) {
         for (int i = 0; i < 16; i++) {
-            mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 8 * i), RA);
-            mbar_init(smem_u32(smem + kFusedSmemBytes + 16 + 16 * 8 + 8 * i), RA);
+            mbar_init(smem_u32(smem + CTL + 16 + 8 * i), RA);
+            mbar_init(smem_u32(smem + CTL + 16 + 16 * 8 + 8 * i), RA);
         }
         if constexpr (ST) {
             mbar_init(mbar, 1);
             *cnt = 0;
         }
         if constexpr (RQ > 0) {
-            for (int i = 0; i < 16; i++) reinterpret_cast<int *>(smem + kFusedSmemBytes + kRingCtlOff)[i] = 0;
-            mbar_init(smem_u32(smem + kFusedSmemBytes + kRingCtlOff + 48), 1);
-            mbar_init(smem_u32(smem + kFusedSmemBytes + kRingCtlOff + 56), 1);
+            for (int i = 0; i < 16; i++) reinterpret_cast<int *>(smem + CTL + kRingCtlOff)[i] = 0;
+            mbar_init(smem_u32(smem + CTL + kRingCtlOff + 48), 1);
+            mbar_init(smem_u32(smem + CTL + kRingCtlOff + 56), 1);
         }
         fence_mbar_init();
         if constexpr (ST) {
@@ -617,7 +657,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     // passes the CTA's arrival on to the global counter, so a step completes at gridDim.x arrivals; the first warp
     // of a CTA that needs a step polls the global counter (one poller per CTA: every acquire load drops the SM's
     // L1) and publishes what it saw in shared memory for the other fifteen.
-    const uint32_t ring_ctl = smem_u32(smem + kFusedSmemBytes + kRingCtlOff);   // +0 ready cnt[4], +16 done cnt[4], +32 seen[2], +40 lock[2], +48 stage mbarrier[2]
+    const uint32_t ring_ctl = smem_u32(smem + CTL + kRingCtlOff);   // +0 ready cnt[4], +16 done cnt[4], +32 seen[2], +40 lock[2], +48 stage mbarrier[2]
     const bool r_staged = RQ > 0 && P.ring_stage != 0;
     const bool r_lean = r_staged && P.L == P.N && gridDim.x >= 16 && (P.c_pitch & 1) == 0;   // see ring_produce_lean_fn
     auto ring_arrive = [&](int which, int step) {       // which: 0 ready (after this warp's stores), 1 done (after its loads)
@@ -712,7 +752,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                 const uint32_t *w = reinterpret_cast<const uint32_t *>(src) + t0;
                 // every other pair through the conversion unit: the steps of the last butterfly stage free one even and
                 // one odd element each, so both forms run side by side
-                if constexpr (e & 1) sc16_pair_to_f32_xu(w[0], w[32], m0, m1, nxr[e], nxi[e]);
+                if constexpr (kB2Dit ? ((e >> 3) & 1) : (e & 1)) sc16_pair_to_f32_xu(w[0], w[32], m0, m1, nxr[e], nxi[e]);
                 else sc16_pair_to_f32(w[0], w[32], m0, m1, nxr[e], nxi[e]);
             } else {
                 const uint2 *w = reinterpret_cast<const uint2 *>(src) + t0;
@@ -769,9 +809,15 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     const int r_ld = r < Rv ? r : Rv - 1;          // ragged last group: recompute a valid gate, never flush it
     const long long gate_off = (long long)P.r0 + (long long)r_ld * P.stride;
     const long long run_off = (long long)P.r0 + (long long)(gg * G) * P.stride;   // first sample of the CTA's run
-    float2 accS[8], accC[8];                       // per last-stage butterfly k of pass B2 (bfly_power)
+    // per last-stage butterfly of pass B2: packed pairs (even e, odd e) per k (bfly_power), or, kB2Dit, accS[k] =
+    // (scalar of e'' = 2k, of e'' = 2k + 1) per output pair (e'', e'' + 16) (bfly_power_halves)
+    float2 accS[8], accC[8];
 #pragma unroll
     for (int j = 0; j < 8; j++) accS[j] = accC[j] = make_float2(0.f, 0.f);
+    auto acc_ref = [&](float2 (&a)[8], auto e_) -> float & {
+        constexpr int e = decltype(e_)::value;
+        if constexpr (e & 1) return a[e / 2].y; else return a[e / 2].x;
+    };
     for (int p = p_lo; p < p_hi; p++) {
         const bool has_next = p + 1 < p_hi || more_tiles;
         const int p_next = p + 1 < p_hi ? p + 1 : 0;
@@ -882,10 +928,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             constexpr int jj = decltype(jj_)::value, f = decltype(f_)::value;
             const int ap = wa + RA * jj;
             if constexpr (X128) {
-                float4 *dst = reinterpret_cast<float4 *>(gate_regions + f * kRegionBytes) + ap * 32 + lane;
+                float4 *dst = reinterpret_cast<float4 *>(gate_regions + f * RB) + ap * 32 + lane;
                 *dst = make_float4(yr.x, yr.y, yi.x, yi.y);
             } else {
-                float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * kRegionBytes) + (ap * 2) * 32 + lane;
+                float2 *dst = reinterpret_cast<float2 *>(gate_regions + f * RB) + (ap * 2) * 32 + lane;
                 dst[0] = yr;
                 dst[32] = yi;
             }
@@ -968,11 +1014,19 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                 const float2 wr = make_float2(cur[4 * k], cur[4 * k + 1]), wi = make_float2(cur[4 * k + 2], cur[4 * k + 3]);
                 const float2 zr = pfma(xr[ph], wr, pneg(pmul(xi[ph], wi)));
                 const float2 zi = pfma(xr[ph], wi, pmul(xi[ph], wr));
-                float *dst = reinterpret_cast<float *>(region + (lane & 15) * (65 * 8) + (lane >> 4) * 4);
-                dst[(c) * 2] = zr.x;
-                dst[(c + 16) * 2] = zr.y;
-                dst[(32 + c) * 2] = zi.x;
-                dst[(32 + c + 16) * 2] = zi.y;
+                if constexpr (kB2Dit) {                              // row (plane, c), column b = lane
+                    float *dst = reinterpret_cast<float *>(region) + lane;
+                    dst[c * 34] = zr.x;
+                    dst[(c + 16) * 34] = zr.y;
+                    dst[(32 + c) * 34] = zi.x;
+                    dst[(32 + c + 16) * 34] = zi.y;
+                } else {
+                    float *dst = reinterpret_cast<float *>(region + (lane & 15) * (65 * 8) + (lane >> 4) * 4);
+                    dst[(c) * 2] = zr.x;
+                    dst[(c + 16) * 2] = zr.y;
+                    dst[(32 + c) * 2] = zi.x;
+                    dst[(32 + c + 16) * 2] = zi.y;
+                }
             });
         });
         __syncwarp();
@@ -985,7 +1039,15 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
         }
         // ---- pass B2: lane = c; decimation-in-frequency radix-32 over b; .x = b, .y = b + 16
         auto b2_front = [&]() {
-            {
+            if constexpr (kB2Dit) {                                  // lane = c: (.x, .y) = (b = 2 j, b = 2 j + 1)
+                const float2 *sr = reinterpret_cast<const float2 *>(reinterpret_cast<const float *>(region) + lane * 34);
+                const float2 *si = reinterpret_cast<const float2 *>(reinterpret_cast<const float *>(region) + (32 + lane) * 34);
+#pragma unroll
+                for (int j = 0; j < 16; j++) {
+                    xr[j] = sr[j];
+                    xi[j] = si[j];
+                }
+            } else {
                 const float2 *src = reinterpret_cast<const float2 *>(region) + lane;
 #pragma unroll
                 for (int bb = 0; bb < 16; bb++) {
@@ -997,11 +1059,15 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                 __syncwarp();
                 if (lane == 0) mbar_arrive(free_base);
             }
-            sfor<0, 16>([&](auto b_) {
-                constexpr int bb = decltype(b_)::value;
-                bfly_dif_halves<bb>(xr[bb], xi[bb]);                 // (.x, .y) -> (even e, odd e) inputs
-            });
-            dft_packed16_head(xr, xi);
+            if constexpr (kB2Dit) {
+                dft_packed<16, 0>(xr, xi);                           // (E[e''], O[e'']) at brev4(e'')
+            } else {
+                sfor<0, 16>([&](auto b_) {
+                    constexpr int bb = decltype(b_)::value;
+                    bfly_dif_halves<bb>(xr[bb], xi[bb]);             // (.x, .y) -> (even e, odd e) inputs
+                });
+                dft_packed16_head(xr, xi);
+            }
         };
         if constexpr (EDM) {
             if (has_next) {                                      // pass B2 with the next window's decode in between
@@ -1011,13 +1077,21 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
                 parity ^= 1u;
                 b2_front();                                      // same basic block as the decode below: the assembler may
                                                                  // start it as early as it finds registers
-                sfor<0, 8>([&](auto k_) {
-                    constexpr int k = decltype(k_)::value;
-                    constexpr int ia = brev<4>(k), ib = brev<4>(k + 8);
-                    bfly_power<2 * k>(xr[ia], xi[ia], xr[ib], xi[ib], accS[k], accC[k]);
-                    ed_dec(std::integral_constant<int, ia>{}, sn, cwn);      // into the registers that just died
-                    ed_dec(std::integral_constant<int, ib>{}, sn, cwn);
-                });
+                if constexpr (kB2Dit) {
+                    sfor<0, 16>([&](auto s_) {
+                        constexpr int e2 = decltype(s_)::value, ph = brev<4>(e2);
+                        bfly_power_halves<e2>(xr[ph], xi[ph], acc_ref(accS, s_), acc_ref(accC, s_));
+                        ed_dec(std::integral_constant<int, ph>{}, sn, cwn);  // into the registers that just died
+                    });
+                } else {
+                    sfor<0, 8>([&](auto k_) {
+                        constexpr int k = decltype(k_)::value;
+                        constexpr int ia = brev<4>(k), ib = brev<4>(k + 8);
+                        bfly_power<2 * k>(xr[ia], xi[ia], xr[ib], xi[ib], accS[k], accC[k]);
+                        ed_dec(std::integral_constant<int, ia>{}, sn, cwn);  // into the registers that just died
+                        ed_dec(std::integral_constant<int, ib>{}, sn, cwn);
+                    });
+                }
                 int p2 = p_next + 1, t2 = tile_next;
                 if (p2 == P.n_ipp) { p2 = 0; t2++; }
                 ed_arrive((p_hi - 1 - p) + left >= 2, t2, p2);
@@ -1029,6 +1103,24 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
         if constexpr (RQ > 0) {
             if (has_next) ring_wait(0, rs + 1);                  // the next window is in the ring (it has been for a while)
         }
+        if constexpr (kB2Dit) {
+            sfor<0, 16>([&](auto s_) {                           // last stage + |X|^2 + accumulate
+                constexpr int e2 = decltype(s_)::value, ph = brev<4>(e2);
+                bfly_power_halves<e2>(xr[ph], xi[ph], acc_ref(accS, s_), acc_ref(accC, s_));
+                if constexpr (PF) {                              // four registers just died: two words of the next window
+                    if constexpr (e2 == 0) {
+                        if constexpr (RQ > 0) pf_next = pf_ring(has_next ? rs + 1 : rs);
+                        else pf_next = has_next ? pf_base(tile_next, p_next) : pf_base(tile, p);
+                    }
+                    sfor<2 * e2, 2 * e2 + 2>([&](auto i_) { pf_load(pf_next, i_); });
+                    if constexpr (e2 == 15) {
+                        if constexpr (!IDC) {
+                            if (bpsk) cw_pf = __ldg(P.Cbits + (long long)(has_next ? p_next : p) * 512 + wa * 32 + lane);
+                        }
+                    }
+                }
+            });
+        } else
         sfor<0, 8>([&](auto k_) {                                // last stage + |X|^2 + accumulate
             constexpr int k = decltype(k_)::value;
             constexpr int ia = brev<4>(k), ib = brev<4>(k + 8);
@@ -1058,6 +1150,14 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     // ---- flush: S_dev[r][q][f_hi = wa][e][c = lane]; other CTAs may hold the rest of this tile's IPPs
     if (r < Rv) {
         float *Srow = P.S + (((long long)r * Q + q) * RA + wa) * 1024 + lane;
+        if constexpr (kB2Dit) {
+            sfor<0, 16>([&](auto s_) {
+                constexpr int e2 = decltype(s_)::value;
+                const float c2 = acc_ref(accC, s_) * pow2w(e2), a = acc_ref(accS, s_);
+                atomicAdd(Srow + e2 * 32, a + c2);
+                atomicAdd(Srow + (e2 + 16) * 32, a - c2);
+            });
+        } else {
         float2 acc[16];                            // acc[j] = (S[e = 2 brev4(j)], S[e + 1]) at k_lo = lane + 32 e
         sfor<0, 8>([&](auto k_) {
             constexpr int k = decltype(k_)::value;
@@ -1071,6 +1171,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             atomicAdd(Srow + e * 32, acc[j].x);
             atomicAdd(Srow + (e + 1) * 32, acc[j].y);
         });
+        }
     }
     }
     };   // run
