@@ -24,7 +24,7 @@
 //
 // Shared memory: 16 regions (one per B warp) of 16*65 8-byte slots + the B1->B2 twiddle table.
 //   A -> B1 :  slot (a'*2 + plane)*32 + b        holds (y[32(2a')+b], y[32(2a'+1)+b]).plane      (STS.64 / LDS.64)
-//              RA = 16: 16-byte slot a'*32 + b   holds both planes of that pair                    (STS.128 / LDS.128)
+//              RA >= 4: 16-byte slot a'*32 + b   holds both planes of that pair                    (STS.128 / LDS.128)
 //   B1 -> B2:  slot  bb*65 + plane*32 + c        holds (z[c][bb], z[c][bb+16]).plane             (STS.32 / LDS.64)
 // Both are free of bank conflicts (the 65 pitch spreads the 4-byte transposed stores over all banks).
 //
@@ -508,9 +508,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     constexpr int LOGRA = ilog2(RA);
     constexpr int FG = RA == 16 ? 4 : 1;   // regions per "full" mbarrier (measured: 4 at RA = 16, 1 below)
     // A -> B1 exchange in 128-bit accesses, slot (a' * 32 + b) of 16 bytes = (y.re pair, y.im pair): half the shared-memory
-    // instructions for the same wavefronts.  Measured: cfg 3 5.974 -> 5.923 ms, paper workload 12.63 -> 12.38 ms; at
-    // RA = 8 and 4 the quad-aligned registers cost spills (cfg 5 28.2 -> 28.5 ms), so those keep the 64-bit layout.
-    constexpr bool X128 = RA == 16;
+    // instructions for the same wavefronts.  Measured: cfg 3 5.974 -> 5.923 ms, paper workload 12.63 -> 12.38 ms.  At
+    // RA = 8 and 4 the register quads cost spills in the kernels of round 1 (cfg 5 28.2 -> 28.5 ms); in the early-decode
+    // kernels they do not (cfg 5 28.13 -> 28.07 ms, cfg 2 0.3427 -> 0.3417 ms).
+    constexpr bool X128 = RA >= 4;
     // Pass B2 as a decimation-in-time radix-32 (pairs = even / odd b) whose last stage -- the one across the two halves
     // of a register pair -- is fused with |X|^2 (bfly_power_halves), instead of the decimation-in-frequency form whose
     // first stage is across the halves: 420 instead of 448 FMA-pipe cycles per thread and window.  Measured: cfg 3
