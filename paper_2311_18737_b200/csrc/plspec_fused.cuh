@@ -853,6 +853,19 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             }
         }
         float2 xr[16], xi[16];
+        if constexpr (IDC) {
+            // N > 16384, step 2: the window the last butterfly stage will fetch is asked into L2 now, a window's time
+            // ahead -- its 128 KB come from the scratch in DRAM, and the register prefetch alone leaves them only the rest
+            // of that stage to arrive (cfg 4 8.70 -> 8.55 ms; the paper workload, which misses L2 one time in ten, does
+            // not gain: 12.12 -> 12.14 ms)
+            if (has_next) {
+                const int rr = group_of(tile_next) * G + g;
+                const unsigned char *wb = reinterpret_cast<const unsigned char *>(P.V) +
+                    ((long long)p_next * P.v_pitch + (long long)P.r0 + (long long)(rr < P.R ? rr : P.R - 1) * P.stride) * ESZ;
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(wb + tid * 128));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(wb + 65536 + tid * 128));
+            }
+        }
         // ---- pass A: load + decode, x[jj*RA + t_hi] = (o = 0, o = 1)
         if constexpr (RQ > 0 || IDC) {                               // decoded already (prefetched from the ring / the scratch)
             sfor<0, RA>([&](auto th_) {
