@@ -506,7 +506,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     constexpr int NJ = 16 / RA;            // a' values per thread in pass A
     constexpr int G = 16 / RA;             // gates per CTA
     constexpr int LOGRA = ilog2(RA);
-    constexpr int FG = RA == 16 ? 4 : 1;   // regions per "full" mbarrier (measured: 4 at RA = 16, 1 below)
+    // regions per "full" mbarrier.  Measured again on the early-decode kernels (profiles/r02b_experiments.md section 13):
+    // RA = 16: 1 / 2 / 4 / 8 -> cfg 3 5.838 / 5.755 / 5.782 / 5.766 ms; RA = 8: 1 / 2 / 4 -> cfg 5 28.06 / 27.68 / 27.75 ms;
+    // RA = 4: 1 / 2 / 4 -> cfg 2 0.3415 / 0.3367 / 0.3467 ms (round 1 had 4 at RA = 16 and 1 below)
+    constexpr int FG = RA >= 4 ? 2 : 1;
     // A -> B1 exchange in 128-bit accesses, slot (a' * 32 + b) of 16 bytes = (y.re pair, y.im pair): half the shared-memory
     // instructions for the same wavefronts.  Measured: cfg 3 5.974 -> 5.923 ms, paper workload 12.63 -> 12.38 ms.  At
     // RA = 8 and 4 the register quads cost spills in the kernels of round 1 (cfg 5 28.2 -> 28.5 ms); in the early-decode
