@@ -596,7 +596,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     // warp of the gate arrives after its last store into the region; the region's owner waits on it before
     // pass B1.  All warps store the regions in the same order f = 0 .. RA - 1, so the owners start pass B one
     // after the other and the stagger carries over to the next window: in steady state nobody waits.  At
-    // RA = 16 four neighbouring regions share one mbarrier (4 arrivals per warp and window instead of 16).
+    // RA >= 4 two neighbouring regions share one mbarrier (FG).
     // free_mbar[gate] (count RA): each owner arrives once it has read its region for the last time in a window
     // (B2 loads done); a pass-A warp waits on it before its first store of the next window (by then the last
     // owner is long past that point, and one probe per window is cheaper than one per region).
