@@ -542,6 +542,34 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     // tile -> gate group and residue
     auto group_of = [&](int t) { return RQ ? t * (int)gridDim.x + (int)blockIdx.x : (Q == 1 ? t : t % P.n_groups); };
     auto resid_of = [&](int t) { return Q == 1 ? 0 : t / P.n_groups; };
+    // ---- ST: stage control.  mbar counts the bytes of one IPP's copy; cnt counts warps done reading it.
+    const uint32_t mbar = smem_u32(smem + CTL);
+    int *const cnt = reinterpret_cast<int *>(smem + CTL + 8);
+    const unsigned char *const stage = smem + CTL + kStageCtlBytes;
+    auto stage_issue = [&](int t, int pp) {                                // one thread: run of tile t, IPP pp
+        const int tg = group_of(t);
+        const int gates_here = (P.R - tg * G) < G ? (P.R - tg * G) : G;
+        const uint32_t run_bytes = (uint32_t)((gates_here - 1) * P.stride + P.L) * ESZ;
+        const long long roff = (long long)P.r0 + (long long)(tg * G) * P.stride;
+        const unsigned char *src = reinterpret_cast<const unsigned char *>(P.V) + ((long long)pp * P.v_pitch + roff) * ESZ;
+        const uint32_t mis = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15);
+        const uint32_t bytes = (mis + run_bytes + 15u) & ~15u;
+        mbar_arrive_expect_tx(mbar, bytes);
+        for (uint32_t off = 0; off < bytes; off += 32768u)
+            bulk_g2s(smem_u32(stage) + off, src - mis + off, (bytes - off) < 32768u ? (bytes - off) : 32768u, mbar);
+    };
+    // the first copy does not depend on anything earlier in the stream (the voltages are the caller's, or were copied
+    // before the launch could start): it is started before the TMEM set-up and the griddepcontrol.wait below, so that its
+    // DRAM latency hides under them
+    if constexpr (ST) {
+        if (tid == 0) {
+            mbar_init(mbar, 1);
+            *cnt = 0;
+            fence_mbar_init();
+            fence_proxy_async();
+            stage_issue(tile0, p0);
+        }
+    }
 
     // ---- twiddles live in tensor memory: every thread re-reads only constants it wrote itself
     //   columns [4 e, 4 e + 4), e = (f - 1) NJ + jj:      pass A -> B1, W_Nk^{t_lo f} for the thread's two t_lo
@@ -576,22 +604,6 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
     unsigned char *const region = smem + warp * RB;                        // this warp's pass-B region
     unsigned char *const gate_regions = smem + (g * RA) * RB;              // regions of this gate (pass A target)
 
-    // ---- ST: stage control.  mbar counts the bytes of one IPP's copy; cnt counts warps done reading it.
-    const uint32_t mbar = smem_u32(smem + CTL);
-    int *const cnt = reinterpret_cast<int *>(smem + CTL + 8);
-    const unsigned char *const stage = smem + CTL + kStageCtlBytes;
-    auto stage_issue = [&](int t, int pp) {                                // one thread: run of tile t, IPP pp
-        const int tg = group_of(t);
-        const int gates_here = (P.R - tg * G) < G ? (P.R - tg * G) : G;
-        const uint32_t run_bytes = (uint32_t)((gates_here - 1) * P.stride + P.L) * ESZ;
-        const long long roff = (long long)P.r0 + (long long)(tg * G) * P.stride;
-        const unsigned char *src = reinterpret_cast<const unsigned char *>(P.V) + ((long long)pp * P.v_pitch + roff) * ESZ;
-        const uint32_t mis = (uint32_t)(reinterpret_cast<uintptr_t>(src) & 15);
-        const uint32_t bytes = (mis + run_bytes + 15u) & ~15u;
-        mbar_arrive_expect_tx(mbar, bytes);
-        for (uint32_t off = 0; off < bytes; off += 32768u)
-            bulk_g2s(smem_u32(stage) + off, src - mis + off, (bytes - off) < 32768u ? (bytes - off) : 32768u, mbar);
-    };
     // Hand-over of the exchange regions without CTA-wide barriers.  full_mbar[region] (count RA): every pass-A
     // warp of the gate arrives after its last store into the region; the region's owner waits on it before
     // pass B1.  All warps store the regions in the same order f = 0 .. RA - 1, so the owners start pass B one
@@ -607,20 +619,12 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             mbar_init(smem_u32(smem + CTL + 16 + 8 * i), RA);
             mbar_init(smem_u32(smem + CTL + 16 + 16 * 8 + 8 * i), RA);
         }
-        if constexpr (ST) {
-            mbar_init(mbar, 1);
-            *cnt = 0;
-        }
         if constexpr (RQ > 0) {
             for (int i = 0; i < 16; i++) reinterpret_cast<int *>(smem + CTL + kRingCtlOff)[i] = 0;
             mbar_init(smem_u32(smem + CTL + kRingCtlOff + 48), 1);
             mbar_init(smem_u32(smem + CTL + kRingCtlOff + 56), 1);
         }
         fence_mbar_init();
-        if constexpr (ST) {
-            fence_proxy_async();
-            stage_issue(tile0, p0);
-        }
     }
     __syncthreads();
     if (RA > 1 && lane == 0) mbar_arrive(free_base);                      // phase 0: the regions start out free
