@@ -758,9 +758,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_kernel(const __grid_co
             const uint32_t m0 = bit_mask<2 * th>(cw[jj]), m1 = bit_mask<2 * th + 1>(cw[jj]);
             if constexpr (DT == DT_SC16) {
                 const uint32_t *w = reinterpret_cast<const uint32_t *>(src) + t0;
-                // every other pair through the conversion unit: the steps of the last butterfly stage free one even and
-                // one odd element each, so both forms run side by side
-                if constexpr (kB2Dit ? ((e >> 3) & 1) : (e & 1)) sc16_pair_to_f32_xu(w[0], w[32], m0, m1, nxr[e], nxi[e]);
+                // some pairs through the conversion unit, spread evenly over the steps of the last butterfly stage, so that
+                // both forms run side by side: every other pair (the steps free one even and one odd element each), or,
+                // where pass B2 is the decimation-in-time form (sixteen steps, element brev4(step)), every fourth
+                // (measured: 1/4, 1/2, 3/4 of the pairs -> cfg 3 5.742 / 5.767 / 5.843 ms, cfg 5 27.79 / 27.69 / 27.88 ms)
+                if constexpr (kB2Dit ? (((e >> 2) & 3) == 3) : (e & 1)) sc16_pair_to_f32_xu(w[0], w[32], m0, m1, nxr[e], nxi[e]);
                 else sc16_pair_to_f32(w[0], w[32], m0, m1, nxr[e], nxi[e]);
             } else {
                 const uint2 *w = reinterpret_cast<const uint2 *>(src) + t0;
